@@ -1,0 +1,92 @@
+"""The per-slice EFIT Picard iteration ("repeatedly performing Picard iterations
+for each time slice"; steps from Sec. II.B-II.D).
+
+Oracle-side (test infrastructure): plain float64, one slice at a time, step by step in the
+order DESIGN.md O7 states:  state = O2;  repeat n_iter times { basis (Eq. 10) -> response
+R = G_P J_b (Eq. 6) -> fit -> node currents -> boundary flux G_B I -> Delta* solve -> add coil
+flux -> search/normalise }.
+"""
+import numpy as np
+from . import basis as _basis, lsq as _lsq, search as _search
+from .gs_solve import GSOperator, boundary_nodes
+
+
+class Device:
+    """Frozen per-device data (the arguments of ptefit_create, include/ptefit.h)."""
+
+    def __init__(self, grid, geom, tables, basis):
+        self.nr, self.nz = grid["nr"], grid["nz"]
+        self.op = GSOperator(self.nr, self.nz, grid["rmin"], grid["rmax"], grid["zmin"], grid["zmax"])
+        self.r, self.z = self.op.r, self.op.z
+        self.dA = self.op.dr * self.op.dz
+        self.sigma = np.asarray(geom["sigma"], np.float64)
+        self.lim_r = np.asarray(geom["lim_r"], np.float64)
+        self.lim_z = np.asarray(geom["lim_z"], np.float64)
+        self.lim_mask = np.asarray(geom["lim_mask"]).astype(bool).reshape(self.nz, self.nr)
+        xm = geom.get("xpt_mask")
+        self.xpt_mask = self.lim_mask if xm is None else np.asarray(xm).astype(bool).reshape(self.nz, self.nr)
+        self.s = int(geom.get("ip_sign", 1))
+        self.cold = (geom["cold_rc"], geom["cold_zc"], geom["cold_a"], geom["cold_b"])
+        N = self.nr * self.nz
+        interior = np.zeros((self.nz, self.nr), bool)
+        interior[1:-1, 1:-1] = True
+        self.interior = interior.ravel()
+        self.gp = np.asarray(tables["gp"], np.float64).reshape(-1, N)
+        self.gc = np.asarray(tables["gc"], np.float64)
+        self.gb = np.asarray(tables["gb"], np.float64).reshape(-1, N)
+        self.ggc = np.asarray(tables["ggc"], np.float64).reshape(N, -1)
+        self.bnd = boundary_nodes(self.nr, self.nz)
+        self.n_p, self.n_ff = basis["n_p"], basis["n_ff"]
+        self.lam = basis.get("lambda_reg", 0.0)
+
+
+def picard_iteration(dev, psin, mask, d, psi_coil):
+    """One Picard iteration from (psin, mask).  Returns dict with X, chi2, status, psi, resp,
+    I (node currents), psi_bdry and the search result `srch` of the new psi."""
+    Jb = _basis.basis_columns(psin, mask, dev.r, dev.dA, dev.n_p, dev.n_ff)     # Eq. 10
+    Jb = Jb.reshape(-1, Jb.shape[-1]) * dev.interior[:, None]                     # edge nodes carry no current
+    resp = dev.gp @ Jb                                                            # Eq. 6: R = G_P J_b
+    X, chi2, st = _lsq.fit(resp, d, dev.sigma, dev.lam)
+    out = dict(X=X, chi2=chi2, status=st, resp=resp)
+    if st != 0:
+        return out
+    I = Jb @ X                                                                    # J_phi dA = J_b X
+    psi_b = dev.gb @ I                                                            # Dirichlet data
+    edge = np.zeros(dev.nr * dev.nz)
+    edge[dev.bnd] = psi_b
+    psi_pl = dev.op.solve_current(I.reshape(dev.nz, dev.nr), edge.reshape(dev.nz, dev.nr))
+    psi = psi_pl + psi_coil
+    srch = _search.search(psi, dev.r, dev.z, dev.lim_mask, dev.xpt_mask, dev.lim_r, dev.lim_z, dev.s)
+    out.update(I=I, psi_bdry=psi_b, psi=psi, srch=srch, status=srch["status"])
+    return out
+
+
+def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False):
+    """ptefit_reconstruct for one slice.  psi0 = None -> cold start (O2), else warm start."""
+    d = np.asarray(b, np.float64) - dev.gc @ np.asarray(ic, np.float64)           # Eq. 2 / Eq. 6 rhs
+    psi_coil = (dev.ggc @ np.asarray(ic, np.float64)).reshape(dev.nz, dev.nr)
+    res = dict(status=0, X=np.zeros(dev.n_p + dev.n_ff), chi2=np.nan, psi=None, srch=None, hist=[])
+    if psi0 is None:
+        psin, mask = _search.cold_start(dev.r, dev.z, dev.lim_mask, *dev.cold)
+        psi = np.zeros((dev.nz, dev.nr))
+        if not mask.any():
+            res["status"] = 1
+    else:
+        psi = np.array(psi0, np.float64).reshape(dev.nz, dev.nr)
+        sr = _search.search(psi, dev.r, dev.z, dev.lim_mask, dev.xpt_mask, dev.lim_r, dev.lim_z, dev.s)
+        res["srch"] = sr
+        res["status"] = sr["status"]
+        psin, mask = sr["psin"], sr["mask"]
+    res["psi"] = psi
+    for it in range(n_iter):
+        if res["status"] != 0:
+            break
+        o = picard_iteration(dev, psin, mask, d, psi_coil)
+        res["X"], res["chi2"], res["status"] = o["X"], o["chi2"], o["status"]
+        if "psi" in o:
+            if trace:
+                res["hist"].append(dict(X=o["X"], chi2=o["chi2"], dpsi=float(np.max(np.abs(o["psi"] - res["psi"]))),
+                                        psi=o["psi"], resp=o["resp"], I=o["I"], psi_bdry=o["psi_bdry"], srch=o["srch"]))
+            res["psi"], res["srch"] = o["psi"], o["srch"]
+            psin, mask = o["srch"]["psin"], o["srch"]["mask"]
+    return res
