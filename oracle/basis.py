@@ -23,3 +23,15 @@ def basis_columns(psin, mask, r, dA, n_p, n_ff):
         cols.append(MU0 / R * (x ** j - x ** n_ff))
     Jb = np.stack(cols, axis=-1) * dA
     return Jb * mask[..., None]
+
+
+def delz_column(Jb_poly, X_prev, nz, nr, dz):
+    """Vertical-shift term (reading O4b; not in the paper, which only notes that the
+    Picard iteration displaces the plasma vertically, PAPER.md:93).  With I' = J_b(psin^k) X^{k-1}
+    the node currents the previous coefficients give on the current flux map,
+    column[j, i] = -(I'[j+1, i] - I'[j-1, i]) / (2 dZ)   (amperes per metre of upward shift),
+    zero on the first and last row.  Jb_poly is [nz*nr, n_p+n_ff]."""
+    Ip = (Jb_poly @ X_prev).reshape(nz, nr)
+    col = np.zeros((nz, nr))
+    col[1:-1, :] = -(Ip[2:, :] - Ip[:-2, :]) / (2.0 * dz)
+    return col.reshape(-1)

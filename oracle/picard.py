@@ -38,13 +38,22 @@ class Device:
         self.bnd = boundary_nodes(self.nr, self.nz)
         self.n_p, self.n_ff = basis["n_p"], basis["n_ff"]
         self.lam = basis.get("lambda_reg", 0.0)
+        self.delz = int(basis.get("delz", 0))          # 1 = append the vertical-shift term
+        self.relax = float(basis.get("relax", 1.0))     # psi^{k+1} = psi^k + relax (psi_new - psi^k)
+        self.nb = self.n_p + self.n_ff + self.delz
 
 
-def picard_iteration(dev, psin, mask, d, psi_coil):
+def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None):
     """One Picard iteration from (psin, mask).  Returns dict with X, chi2, status, psi, resp,
-    I (node currents), psi_bdry and the search result `srch` of the new psi."""
+    I (node currents), psi_bdry and the search result `srch` of the new psi.
+    X_prev: previous coefficients (for the delz column); psi_prev: flux to relax towards/from
+    (None = take the new flux as is)."""
     Jb = _basis.basis_columns(psin, mask, dev.r, dev.dA, dev.n_p, dev.n_ff)     # Eq. 10
     Jb = Jb.reshape(-1, Jb.shape[-1]) * dev.interior[:, None]                     # edge nodes carry no current
+    if dev.delz:
+        xp = np.zeros(dev.n_p + dev.n_ff) if X_prev is None else np.asarray(X_prev)[:dev.n_p + dev.n_ff]
+        col = _basis.delz_column(Jb, xp, dev.nz, dev.nr, dev.op.dz) * dev.interior
+        Jb = np.concatenate([Jb, col[:, None]], axis=1)
     resp = dev.gp @ Jb                                                            # Eq. 6: R = G_P J_b
     X, chi2, st = _lsq.fit(resp, d, dev.sigma, dev.lam)
     out = dict(X=X, chi2=chi2, status=st, resp=resp)
@@ -56,6 +65,8 @@ def picard_iteration(dev, psin, mask, d, psi_coil):
     edge[dev.bnd] = psi_b
     psi_pl = dev.op.solve_current(I.reshape(dev.nz, dev.nr), edge.reshape(dev.nz, dev.nr))
     psi = psi_pl + psi_coil
+    if psi_prev is not None:
+        psi = psi_prev + dev.relax * (psi - psi_prev)
     srch = _search.search(psi, dev.r, dev.z, dev.lim_mask, dev.xpt_mask, dev.lim_r, dev.lim_z, dev.s)
     out.update(I=I, psi_bdry=psi_b, psi=psi, srch=srch, status=srch["status"])
     return out
@@ -65,7 +76,7 @@ def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False):
     """ptefit_reconstruct for one slice.  psi0 = None -> cold start (O2), else warm start."""
     d = np.asarray(b, np.float64) - dev.gc @ np.asarray(ic, np.float64)           # Eq. 2 / Eq. 6 rhs
     psi_coil = (dev.ggc @ np.asarray(ic, np.float64)).reshape(dev.nz, dev.nr)
-    res = dict(status=0, X=np.zeros(dev.n_p + dev.n_ff), chi2=np.nan, psi=None, srch=None, hist=[])
+    res = dict(status=0, X=np.zeros(dev.nb), chi2=np.nan, psi=None, srch=None, hist=[])
     if psi0 is None:
         psin, mask = _search.cold_start(dev.r, dev.z, dev.lim_mask, *dev.cold)
         psi = np.zeros((dev.nz, dev.nr))
@@ -81,7 +92,9 @@ def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False):
     for it in range(n_iter):
         if res["status"] != 0:
             break
-        o = picard_iteration(dev, psin, mask, d, psi_coil)
+        have_prev = (psi0 is not None) or it > 0     # cold start: the first flux is taken as is
+        o = picard_iteration(dev, psin, mask, d, psi_coil, X_prev=res["X"],
+                             psi_prev=res["psi"] if have_prev else None)
         res["X"], res["chi2"], res["status"] = o["X"], o["chi2"], o["status"]
         if "psi" in o:
             if trace:

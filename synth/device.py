@@ -25,6 +25,7 @@ CONFIGS = {
 }
 RMIN, RMAX = 0.15, 1.60
 LAMBDA_REG = 0.01
+RELAX = 0.6
 
 
 def filament_psi(a, zs, rho, zf):
@@ -131,7 +132,7 @@ def make_device(name, with_tables=True):
                 cold_rc=0.80, cold_zc=0.0, cold_a=0.40, cold_b=0.72)
     meta = dict(cfg=c, name=name, r=r, z=z, sen_r=sen_r, sen_z=sen_z, alpha=alpha, n_probe=c["n_probe"],
                 src_r=src_r, src_z=src_z, src_w=src_w, n_pf=c["n_pf"])
-    out = dict(grid=grid, geom=geom, basis=dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=LAMBDA_REG),
+    out = dict(grid=grid, geom=geom, basis=dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=LAMBDA_REG, delz=1, relax=RELAX),
                meta=meta, tables=None)
     if with_tables:
         out["tables"] = make_tables(meta, grid)
