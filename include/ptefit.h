@@ -1,0 +1,150 @@
+/* ptefit.h -- C ABI of the B200-native PTEFIT hot path (arxiv 2601.12378).
+ *
+ * The library runs the per-time-slice EFIT Picard iteration of PTEFIT on one GPU (sm_100a):
+ *   basis J_b (Eq. 8-11) -> response R = G_P J_b (Eq. 6)
+ *   -> least squares for X -> node currents J_b X -> boundary flux G_B I
+ *   -> Delta* psi = -mu0 R J_phi by DST-in-Z + tridiagonal-in-R (Eq. 1, 118-120)
+ *   -> axis / X-point / LCFS search and normalisation (Sec. II.D).
+ * It never computes Green's functions (PAPER.md:65-79 is an offline precompute): the tables are
+ * inputs of ptefit_create.  There is no CPU fallback: every entry point fails with
+ * PTEFIT_ERR_CUDA when no sm_100 device is usable.
+ *
+ * Conventions: COCOS 7, psi is flux per radian; grid node (i, j) has
+ * R_i = rmin + i dR, Z_j = zmin + j dZ and flat index n = j*nr + i (R fastest).
+ * All matrices are row-major.  "real" = float (PTEFIT_FP32) or double (PTEFIT_FP64).
+ */
+#ifndef PTEFIT_H
+#define PTEFIT_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ptefit_handle ptefit_handle; /* opaque; owns every device copy it makes */
+
+typedef enum {
+  PTEFIT_OK = 0,
+  PTEFIT_ERR_INVALID_ARG = 1,
+  PTEFIT_ERR_UNSUPPORTED = 2,
+  PTEFIT_ERR_CUDA = 3,
+  PTEFIT_ERR_NOMEM = 4
+} ptefit_status;
+
+typedef enum { PTEFIT_FP32 = 0, PTEFIT_FP64 = 1 } ptefit_precision;
+/* Arithmetic of the two dense contractions (R = G_P J_b and psi_bdry = G_B I) in FP32 mode:
+ * 3xTF32 = error-compensated tensor-core products (FP32-accurate), TF32 = single pass,
+ * FFMA = plain FP32 FMA.  FP64 mode always uses FP64 arithmetic. */
+typedef enum { PTEFIT_GEMM_3XTF32 = 0, PTEFIT_GEMM_TF32 = 1, PTEFIT_GEMM_FFMA = 2 } ptefit_gemm_mode;
+
+/* Grid.  nz-1 must be a power of two in [8, 256] (DST length); nr in [5, 257]. */
+typedef struct { int nr, nz; double rmin, rmax, zmin, zmax; } ptefit_grid;
+
+/* Geometry.  All pointers are HOST memory, read during ptefit_create only. */
+typedef struct {
+  int n_meas;                     /* M: magnetic probes + flux loops (rows of Eq. 2)            */
+  int n_coil;                     /* n_c: PF coils + eddy filaments (columns of G_C)            */
+  const double *sigma;            /* [n_meas] 1-sigma of each channel, > 0 (fit weights 1/sigma)*/
+  int n_lim;                      /* limiter polygon vertices, 1..256            */
+  const double *lim_r, *lim_z;    /* [n_lim] inside the grid rectangle                          */
+  const unsigned char *lim_mask;  /* [nz*nr] 1 = node may carry plasma; never an edge node      */
+  const unsigned char *xpt_mask;  /* [nz*nr] 1 = node may host an X-point; NULL = lim_mask      */
+  int ip_sign;                    /* +1 or -1: sign of the plasma current                       */
+  double cold_rc, cold_zc, cold_a, cold_b; /* cold-start ellipse (warm_start = 0)               */
+} ptefit_geometry;
+
+/* Green's tables, HOST, FP64, row-major.  Columns of gp/gb that belong to edge nodes are ignored
+ * (edge nodes never carry current).  Boundary-node order k of gb: bottom row j=0 (i=0..nr-1), top
+ * row j=nz-1 (i=0..nr-1), left column i=0 (j=1..nz-2), right column i=nr-1 (j=1..nz-2). */
+typedef struct {
+  const double *gp;   /* [n_meas][nz*nr] response of channel m per ampere at node n (Eq. 2 G_P) */
+  const double *gc;   /* [n_meas][n_coil] (Eq. 2 G_C)                                           */
+  const double *gb;   /* [n_bnd][nz*nr]  flux/rad at boundary node k per ampere at node n       */
+  const double *ggc;  /* [nz*nr][n_coil] flux/rad at node n per unit coil current               */
+} ptefit_tables;
+
+/* One basis term (a column of J_b, Eq. 10).  kind 0: P' term  R (x^i - x^N) dA;
+ * kind 1: FF' term (mu0/R)(x^i - x^N) dA;  kind 2: vertical-shift term -dI'/dZ (DESIGN.md
+ * reading O4b; i, N ignored; must be the last term, at most one).  x = normalised flux. */
+typedef struct { int kind; int i; int N; } ptefit_term;
+
+typedef struct {
+  int n_terms;                 /* 1..12                                                         */
+  const ptefit_term *terms;    /* HOST                                                          */
+  double lambda_reg;           /* Tikhonov weight in equilibrated coordinates; 0 = Eq. 6 as is  */
+  double relax;                /* psi^{k+1} = psi^k + relax (psi_new - psi^k); 1 = plain Picard */
+} ptefit_basis;
+
+typedef struct {
+  ptefit_precision precision;
+  ptefit_gemm_mode gemm;
+  int max_batch;               /* largest batch ptefit_reconstruct will be called with          */
+} ptefit_options;
+
+/* Build a reconstruction handle: validates, copies the tables to the device (rounded to nearest
+ * FP32 in FP32 mode), precomputes the DST/tridiagonal factors, allocates all workspaces for
+ * max_batch slices.  The caller keeps ownership of everything it passes.  Synchronous.
+ * On error *out = NULL and ptefit_global_error() describes the failure. */
+ptefit_status ptefit_create(const ptefit_grid *grid, const ptefit_geometry *geom,
+                            const ptefit_tables *tables, const ptefit_basis *basis,
+                            const ptefit_options *opts, ptefit_handle **out);
+
+/* Reconstruct `batch` independent time slices (1 <= batch <= max_batch), n_iter Picard
+ * iterations each.  Every d_* pointer is caller-owned DEVICE memory; `real` per precision.
+ * Asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream); no host
+ * synchronisation, no allocation.  Outputs that are NULL are skipped (d_psi, d_coeffs required).
+ * Numerical failure of a slice is reported in d_status[slice] and never aborts the batch:
+ * 0 ok, 1 plasma lost, 2 non-finite, 3 singular fit, 4 more than 32 X-point candidates.
+ * After a failure the slice's other outputs are unspecified. */
+ptefit_status ptefit_reconstruct(ptefit_handle *h, int batch,
+    const void *d_b,        /* [batch][n_meas]  real: measurements b (Eq. 2)                    */
+    const void *d_ic,       /* [batch][n_coil]  real: coil + eddy currents I_C                  */
+    int n_iter, int warm_start, /* warm_start = 1: d_psi holds the starting flux                */
+    void *d_psi,            /* [batch][nz][nr]  real, in/out: poloidal flux per radian          */
+    void *d_coeffs,         /* [batch][n_terms] real: X of the last fit (Eq. 11)                */
+    int *d_axis_ij,         /* [batch][2] (i, j) of the axis node                               */
+    void *d_axis_rzpsi,     /* [batch][3] real: refined (R, Z, psi) of the axis                 */
+    int *d_xpt_ij,          /* [batch][2] best X-point candidate node, (-1,-1) if none          */
+    void *d_xpt_rzpsi,      /* [batch][3] real                                                  */
+    void *d_psi_bnd,        /* [batch] real: LCFS flux                                          */
+    int *d_limited,         /* [batch] 1 = boundary defined by a limiter vertex                 */
+    void *d_chi2,           /* [batch] real: chi^2 of the last fit                              */
+    int *d_status,          /* [batch]                                                          */
+    void *cuda_stream);
+
+/* Same as ptefit_reconstruct but every buffer is HOST memory (pageable or pinned): the call
+ * copies inputs to the device, runs, copies every non-NULL output back and synchronises. */
+ptefit_status ptefit_reconstruct_host(ptefit_handle *h, int batch,
+    const void *b, const void *ic, int n_iter, int warm_start, void *psi, void *coeffs,
+    int *axis_ij, void *axis_rzpsi, int *xpt_ij, void *xpt_rzpsi, void *psi_bnd, int *limited,
+    void *chi2, int *status);
+
+/* Test hooks (lock-step parity, tests/): run single stages on caller DEVICE buffers. */
+/* Delta* solve: psi[batch][nz][nr] = solve(-mu0 R I/dA with edge data psi_bdry[batch][n_bnd]). */
+ptefit_status ptefit_debug_gs_solve(ptefit_handle *h, int batch, const void *d_I /*[batch][nz*nr]*/,
+                                    const void *d_psi_bdry, void *d_psi_out, void *cuda_stream);
+/* Search: from d_psi fills the handle's internal state and writes xn[batch][nz*nr]
+ * (normalised flux in the mask, -1 outside) and the search outputs as in ptefit_reconstruct. */
+ptefit_status ptefit_debug_search(ptefit_handle *h, int batch, const void *d_psi, void *d_xn,
+    int *d_axis_ij, void *d_axis_rzpsi, int *d_xpt_ij, void *d_xpt_rzpsi, void *d_psi_bnd,
+    int *d_limited, int *d_status, void *cuda_stream);
+/* Response + fit from xn: resp[batch][n_meas][n_terms], coeffs, chi2 (X_prev = d_xprev or 0). */
+ptefit_status ptefit_debug_fit(ptefit_handle *h, int batch, const void *d_xn, const void *d_b,
+    const void *d_ic, const void *d_xprev, void *d_resp, void *d_coeffs, void *d_chi2,
+    int *d_status, void *cuda_stream);
+
+/* Number of kernel launches the last ptefit_reconstruct enqueued (bench.py's gpu_launches). */
+int ptefit_last_launch_count(const ptefit_handle *h);
+/* Device time in ms of the stages of the last reconstruct call when profiling was enabled by
+ * ptefit_set_profiling(h, 1): out[0..5] = setup, response, lsq, boundary, solve, search (sums
+ * over iterations).  Profiling inserts events only; returns PTEFIT_ERR_INVALID_ARG if disabled.
+ * Synchronises the stream. */
+ptefit_status ptefit_set_profiling(ptefit_handle *h, int on);
+ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
+
+void ptefit_destroy(ptefit_handle *h);
+const char *ptefit_last_error(const ptefit_handle *h);
+const char *ptefit_global_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTEFIT_H */
