@@ -1,0 +1,246 @@
+// ptefit.cu -- C ABI (include/ptefit.h) of the B200-native PTEFIT Picard iteration.
+// Host side: validation, table upload, DST/tridiagonal factor precompute, launch sequence.
+// No CPU compute path exists: without a usable device every entry point returns PTEFIT_ERR_CUDA.
+#include "../../include/ptefit.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "fit_kernels.cuh"
+#include "search_kernels.cuh"
+#include "solve_kernels.cuh"
+
+using namespace ptefit;
+
+static thread_local std::string g_error;
+
+struct ptefit_handle {
+  ptefit_precision prec;
+  ptefit_gemm_mode gemm;
+  int max_batch;
+  Dev<float> d32;
+  Dev<double> d64;
+  std::vector<void *> allocs;
+  std::string error;
+  int launches = 0;
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev;          // stage boundaries of the last call
+  std::vector<int> ev_stage;
+  // staging buffers of ptefit_reconstruct_host
+  void *hb = nullptr, *hic = nullptr, *hpsi = nullptr, *hco = nullptr, *hax = nullptr, *hxp = nullptr,
+       *hpb = nullptr, *hchi = nullptr;
+  int *haxij = nullptr, *hxpij = nullptr, *hlim = nullptr, *hst = nullptr;
+  cudaStream_t hstream = nullptr;
+};
+
+#define CK(call)                                                                          \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      char buf_[512];                                                                     \
+      snprintf(buf_, sizeof buf_, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+      if (h) h->error = buf_;                                                             \
+      g_error = buf_;                                                                     \
+      return e_ == cudaErrorMemoryAllocation ? PTEFIT_ERR_NOMEM : PTEFIT_ERR_CUDA;        \
+    }                                                                                     \
+  } while (0)
+
+static ptefit_status fail(ptefit_handle *h, ptefit_status st, const char *msg) {
+  g_error = msg;
+  if (h) h->error = msg;
+  return st;
+}
+
+template <typename T>
+static ptefit_status dev_alloc(ptefit_handle *h, T **p, size_t count) {
+  void *q = nullptr;
+  CK(cudaMalloc(&q, count * sizeof(T) + 256));
+  CK(cudaMemset(q, 0, count * sizeof(T) + 256));
+  h->allocs.push_back(q);
+  *p = reinterpret_cast<T *>(q);
+  return PTEFIT_OK;
+}
+
+template <typename T, typename S>
+static ptefit_status upload(ptefit_handle *h, const T **p, const S *src, size_t count) {
+  std::vector<T> tmp(count);
+  for (size_t k = 0; k < count; ++k) tmp[k] = (T)src[k];   // round to nearest (FP32 mode)
+  T *q = nullptr;
+  ptefit_status st = dev_alloc(h, &q, count);
+  if (st != PTEFIT_OK) return st;
+  CK(cudaMemcpy(q, tmp.data(), count * sizeof(T), cudaMemcpyHostToDevice));
+  *p = q;
+  return PTEFIT_OK;
+}
+
+#define TRY(x)                        \
+  do {                                \
+    ptefit_status st_ = (x);          \
+    if (st_ != PTEFIT_OK) return st_; \
+  } while (0)
+
+template <typename T>
+static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, const ptefit_geometry *ge,
+                           const ptefit_tables *tb, const ptefit_basis *ba, int B) {
+  D.nr = g->nr; D.nz = g->nz; D.N = g->nr * g->nz; D.nri = g->nr - 2; D.nzi = g->nz - 2;
+  D.nbnd = 2 * (g->nr + g->nz) - 4; D.M = ge->n_meas; D.nc = ge->n_coil; D.nt = ba->n_terms;
+  D.nlim = ge->n_lim; D.ip_sign = ge->ip_sign;
+  D.rmin = g->rmin; D.zmin = g->zmin;
+  D.dr = (g->rmax - g->rmin) / (g->nr - 1); D.dz = (g->zmax - g->zmin) / (g->nz - 1);
+  D.dA = D.dr * D.dz; D.lambda_reg = ba->lambda_reg; D.relax = ba->relax;
+  D.cold_rc = ge->cold_rc; D.cold_zc = ge->cold_zc; D.cold_a = ge->cold_a; D.cold_b = ge->cold_b;
+  D.npoly = 0; D.has_delz = 0;
+  for (int l = 0; l < ba->n_terms; ++l) {
+    D.terms[l].kind = ba->terms[l].kind; D.terms[l].i = ba->terms[l].i; D.terms[l].N = ba->terms[l].N;
+    if (ba->terms[l].kind == 2) D.has_delz = 1; else D.npoly++;
+  }
+  const size_t N = D.N;
+  // tables; edge-node columns of gp / gb are zeroed (edge nodes never carry current)
+  {
+    std::vector<double> t(tb->gp, tb->gp + (size_t)D.M * N);
+    std::vector<double> u(tb->gb, tb->gb + (size_t)D.nbnd * N);
+    for (int j = 0; j < D.nz; ++j)
+      for (int i = 0; i < D.nr; ++i)
+        if (i == 0 || j == 0 || i == D.nr - 1 || j == D.nz - 1) {
+          for (int m = 0; m < D.M; ++m) t[(size_t)m * N + j * D.nr + i] = 0.0;
+          for (int k = 0; k < D.nbnd; ++k) u[(size_t)k * N + j * D.nr + i] = 0.0;
+        }
+    TRY(upload(h, &D.gp, t.data(), t.size()));
+    TRY(upload(h, &D.gb, u.data(), u.size()));
+  }
+  TRY(upload(h, &D.gc, tb->gc, (size_t)D.M * D.nc));
+  TRY(upload(h, &D.ggc, tb->ggc, N * D.nc));
+  {
+    std::vector<double> w(D.M);
+    for (int m = 0; m < D.M; ++m) w[m] = 1.0 / ge->sigma[m];
+    TRY(upload(h, &D.inv_sigma, w.data(), w.size()));
+  }
+  TRY(upload(h, &D.lim_mask, ge->lim_mask, N));
+  TRY(upload(h, &D.xpt_mask, ge->xpt_mask ? ge->xpt_mask : ge->lim_mask, N));
+  TRY(upload(h, &D.lim_r, ge->lim_r, (size_t)D.nlim));
+  TRY(upload(h, &D.lim_z, ge->lim_z, (size_t)D.nlim));
+  // Delta* factors ("the coefficient matrices can be pre-computed"): for each DST
+  // mode m the tridiagonal [cw_i, -2/dR^2 + lam_m, ce_i] is LU-factored in FP64 on the host.
+  {
+    const int nri = D.nri, nzi = D.nzi;
+    std::vector<double> w((size_t)nri * nzi), ib((size_t)nri * nzi), ce(nri), cw(nri);
+    for (int i = 0; i < nri; ++i) {
+      const double R = D.rmin + (i + 1) * D.dr;
+      cw[i] = (1.0 + D.dr / (2.0 * R)) / (D.dr * D.dr);
+      ce[i] = (1.0 - D.dr / (2.0 * R)) / (D.dr * D.dr);
+    }
+    const double pi = 3.14159265358979323846;
+    for (int mm = 0; mm < nzi; ++mm) {
+      const double sn = sin(pi * (mm + 1) / (2.0 * (D.nz - 1)));
+      const double diag = -2.0 / (D.dr * D.dr) - 4.0 / (D.dz * D.dz) * sn * sn;
+      double piv = diag;
+      w[mm] = 0.0; ib[mm] = 1.0 / piv;
+      for (int i = 1; i < nri; ++i) {
+        const double wi = cw[i] / piv;
+        piv = diag - wi * ce[i - 1];
+        w[(size_t)i * nzi + mm] = wi;
+        ib[(size_t)i * nzi + mm] = 1.0 / piv;
+      }
+    }
+    ce[nri - 1] = ce[nri - 1];  // multiplies x_{nri} = 0 in the back substitution
+    TRY(upload(h, &D.tri_w, w.data(), w.size()));
+    TRY(upload(h, &D.tri_invb, ib.data(), ib.size()));
+    TRY(upload(h, &D.tri_ce, ce.data(), ce.size()));
+    const int period = 2 * (D.nz - 1);
+    std::vector<double> st(period);
+    for (int k = 0; k < period; ++k) st[k] = sin(pi * k / (D.nz - 1));
+    st[D.nz - 1] = 0.0;
+    TRY(upload(h, &D.sintab, st.data(), st.size()));
+  }
+  // workspaces
+  TRY(dev_alloc(h, &D.xn, (size_t)B * N));
+  TRY(dev_alloc(h, &D.psi_coil, (size_t)B * N));
+  TRY(dev_alloc(h, &D.dred, (size_t)B * D.M));
+  TRY(dev_alloc(h, &D.resp, (size_t)B * D.M * D.nt));
+  TRY(dev_alloc(h, &D.cur, (size_t)B * N));
+  TRY(dev_alloc(h, &D.dzc, (size_t)B * N));
+  TRY(dev_alloc(h, &D.psi_bdry, (size_t)B * D.nbnd));
+  TRY(dev_alloc(h, &D.fhat, (size_t)B * D.nri * D.nzi));
+  TRY(dev_alloc(h, &D.ytmp, (size_t)B * D.nri * D.nzi));
+  TRY(dev_alloc(h, &D.X, (size_t)B * D.nt));
+  TRY(dev_alloc(h, &D.Xprev, (size_t)B * D.nt));
+  TRY(dev_alloc(h, &D.chi2, (size_t)B));
+  TRY(dev_alloc(h, &D.so, (size_t)B));
+  TRY(dev_alloc(h, &D.status, (size_t)B));
+  return PTEFIT_OK;
+}
+
+extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geometry *ge,
+                                       const ptefit_tables *tb, const ptefit_basis *ba,
+                                       const ptefit_options *op, ptefit_handle **out) {
+  ptefit_handle *h = nullptr;
+  if (out) *out = nullptr;
+  if (!g || !ge || !tb || !ba || !op || !out) return fail(h, PTEFIT_ERR_INVALID_ARG, "null argument");
+  int p2 = g->nz - 1;
+  if (g->nz < 9 || g->nz > 257 || (p2 & (p2 - 1)) != 0) return fail(h, PTEFIT_ERR_INVALID_ARG, "nz-1 must be a power of two in [8,256]");
+  if (g->nr < 5 || g->nr > 257) return fail(h, PTEFIT_ERR_INVALID_ARG, "nr must be in [5,257]");
+  if (!(g->rmin > 0.0) || !(g->rmax > g->rmin) || !(g->zmax > g->zmin)) return fail(h, PTEFIT_ERR_INVALID_ARG, "bad grid extents");
+  if (ge->n_meas < 1 || ge->n_coil < 1 || ge->n_coil > 1024 || !ge->sigma || !ge->lim_mask || !ge->lim_r || !ge->lim_z)
+    return fail(h, PTEFIT_ERR_INVALID_ARG, "bad geometry");
+  if (ge->n_lim < 1 || ge->n_lim > PTEFIT_MAX_LIM) return fail(h, PTEFIT_ERR_INVALID_ARG, "n_lim must be in [1,256]");
+  if (ge->ip_sign != 1 && ge->ip_sign != -1) return fail(h, PTEFIT_ERR_INVALID_ARG, "ip_sign must be +-1");
+  if (!(ge->cold_a > 0.0) || !(ge->cold_b > 0.0)) return fail(h, PTEFIT_ERR_INVALID_ARG, "bad cold-start ellipse");
+  for (int m = 0; m < ge->n_meas; ++m)
+    if (!(ge->sigma[m] > 0.0)) return fail(h, PTEFIT_ERR_INVALID_ARG, "sigma must be > 0");
+  for (int v = 0; v < ge->n_lim; ++v)
+    if (ge->lim_r[v] < g->rmin || ge->lim_r[v] > g->rmax || ge->lim_z[v] < g->zmin || ge->lim_z[v] > g->zmax)
+      return fail(h, PTEFIT_ERR_INVALID_ARG, "limiter vertex outside the grid");
+  for (int j = 0; j < g->nz; ++j)
+    for (int i = 0; i < g->nr; ++i)
+      if (i == 0 || j == 0 || i == g->nr - 1 || j == g->nz - 1) {
+        if (ge->lim_mask[j * g->nr + i] || (ge->xpt_mask && ge->xpt_mask[j * g->nr + i]))
+          return fail(h, PTEFIT_ERR_INVALID_ARG, "lim_mask / xpt_mask must be 0 on edge nodes");
+      }
+  if (!tb->gp || !tb->gc || !tb->gb || !tb->ggc) return fail(h, PTEFIT_ERR_INVALID_ARG, "null table");
+  if (ba->n_terms < 1 || ba->n_terms > PTEFIT_MAX_TERMS || !ba->terms) return fail(h, PTEFIT_ERR_INVALID_ARG, "n_terms must be in [1,12]");
+  for (int l = 0; l < ba->n_terms; ++l) {
+    const ptefit_term &t = ba->terms[l];
+    if (t.kind < 0 || t.kind > 2) return fail(h, PTEFIT_ERR_UNSUPPORTED, "unknown basis term kind");
+    if (t.kind == 2 && l != ba->n_terms - 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "the vertical-shift term must be last");
+    if (t.kind != 2 && (t.i < 0 || t.N <= t.i || t.N > 8)) return fail(h, PTEFIT_ERR_INVALID_ARG, "term exponents need 0 <= i < N <= 8");
+  }
+  if (ba->n_terms == 1 && ba->terms[0].kind == 2) return fail(h, PTEFIT_ERR_INVALID_ARG, "need at least one P'/FF' term");
+  if (!(ba->lambda_reg >= 0.0) || !(ba->relax > 0.0) || ba->relax > 1.0) return fail(h, PTEFIT_ERR_INVALID_ARG, "need lambda_reg >= 0 and 0 < relax <= 1");
+  if (op->max_batch < 1 || op->max_batch > 65535) return fail(h, PTEFIT_ERR_INVALID_ARG, "max_batch must be in [1,65535]");
+  if (op->precision != PTEFIT_FP32 && op->precision != PTEFIT_FP64) return fail(h, PTEFIT_ERR_INVALID_ARG, "bad precision");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(h, PTEFIT_ERR_CUDA, "no CUDA device (there is no CPU fallback)");
+  {
+    int dev = 0, major = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (major != 10) return fail(h, PTEFIT_ERR_CUDA, "device is not sm_100 (the library is built for sm_100a only)");
+  }
+  h = new ptefit_handle();
+  h->prec = op->precision; h->gemm = op->gemm; h->max_batch = op->max_batch;
+  ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
+                                              : build(h, h->d64, g, ge, tb, ba, op->max_batch);
+  if (st != PTEFIT_OK) { std::string e = h->error; ptefit_destroy(h); g_error = e; return st; }
+  *out = h;
+  return PTEFIT_OK;
+}
+
+extern "C" void ptefit_destroy(ptefit_handle *h) {
+  if (!h) return;
+  for (void *p : h->allocs) cudaFree(p);
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+  void *hp[] = {h->hb, h->hic, h->hpsi, h->hco, h->hax, h->hxp, h->hpb, h->hchi, h->haxij, h->hxpij, h->hlim, h->hst};
+  for (void *p : hp) if (p) cudaFree(p);
+  if (h->hstream) cudaStreamDestroy(h->hstream);
+  delete h;
+}
+
+extern "C" const char *ptefit_last_error(const ptefit_handle *h) { return h ? h->error.c_str() : g_error.c_str(); }
+extern "C" const char *ptefit_global_error(void) { return g_error.c_str(); }
+extern "C" int ptefit_last_launch_count(const ptefit_handle *h) { return h ? h->launches : 0; }
+
+#include "launch.inc"

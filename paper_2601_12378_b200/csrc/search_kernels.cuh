@@ -1,0 +1,205 @@
+// search_kernels.cuh -- A1/A9: magnetic axis, X-point candidates, limiter fluxes, boundary flux,
+// plasma mask and normalised flux (Sec. II.D; rules per DESIGN.md reading O3).
+// One CTA per slice; all fit arithmetic in FP64 on the T-typed flux so that classification
+// decisions (det < 0, |x*| <= 1/2) are taken in the same precision on both code paths.
+#pragma once
+#include "common.cuh"
+
+namespace ptefit {
+
+constexpr int SEARCH_THREADS = 512;
+
+struct Fit { double det, xs, ys, ps; };
+
+// 3x3 least-squares quadratic with the pre-inverted normal equations: integer
+// weight table, index units.  p points at the centre node, ld = nr.
+template <typename T>
+__device__ __forceinline__ Fit quad_fit(const T *__restrict__ p, int ld) {
+  const double a = p[-ld - 1], b = p[-ld], c = p[-ld + 1];
+  const double d = p[-1], e = p[0], f = p[1];
+  const double g = p[ld - 1], h = p[ld], k = p[ld + 1];
+  const double cx = ((c + f + k) - (a + d + g)) * (1.0 / 6.0);
+  const double cy = ((g + h + k) - (a + b + c)) * (1.0 / 6.0);
+  const double cxx = ((a + d + g) - 2.0 * (b + e + h) + (c + f + k)) * (1.0 / 6.0);
+  const double cyy = ((a + b + c) - 2.0 * (d + e + f) + (g + h + k)) * (1.0 / 6.0);
+  const double cxy = (k + a - g - c) * 0.25;
+  const double c0 = (5.0 * e + 2.0 * (b + d + f + h) - (a + c + g + k)) * (1.0 / 9.0);
+  Fit o;
+  o.det = 4.0 * cxx * cyy - cxy * cxy;
+  o.xs = -(2.0 * cyy * cx - cxy * cy) / o.det;
+  o.ys = -(2.0 * cxx * cy - cxy * cx) / o.det;
+  o.ps = c0 + 0.5 * (cx * o.xs + cy * o.ys);
+  return o;
+}
+
+struct ArgMax { double v; int n; };
+__device__ __forceinline__ ArgMax better(ArgMax a, ArgMax b) {   // larger v, tie -> smaller n
+  return (b.v > a.v || (b.v == a.v && b.n < a.n)) ? b : a;
+}
+__device__ __forceinline__ ArgMax block_argmax(ArgMax a, ArgMax *sh) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ArgMax b;
+    b.v = __shfl_xor_sync(0xffffffffu, a.v, o);
+    b.n = __shfl_xor_sync(0xffffffffu, a.n, o);
+    a = better(a, b);
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  __syncthreads();
+  if (lane == 0) sh[w] = a;
+  __syncthreads();
+  ArgMax r = sh[0];
+  for (int k = 1; k < SEARCH_THREADS / 32; ++k) r = better(r, sh[k]);
+  return r;
+}
+
+// grid B, block SEARCH_THREADS.  Reads psi[s], writes xn[s] (normalised flux in the mask, -1
+// outside), D.so[s] and D.status[s] (sticky).
+template <typename T>
+__global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__restrict__ psi_all,
+                                                            T *__restrict__ xn_all) {
+  const int s = blockIdx.x;
+  const T *psi = psi_all + (size_t)s * D.N;
+  T *xn = xn_all + (size_t)s * D.N;
+  const int nr = D.nr, N = D.N;
+  const double sg = (double)D.ip_sign;
+  __shared__ ArgMax sh_am[SEARCH_THREADS / 32];
+  __shared__ int sh_flag, sh_ncand, sh_count;
+  __shared__ double cR[PTEFIT_MAX_CAND], cZ[PTEFIT_MAX_CAND], cP[PTEFIT_MAX_CAND];
+  __shared__ int cN[PTEFIT_MAX_CAND];
+  __shared__ SearchOut so;
+  __shared__ int sh_status;
+  if (threadIdx.x == 0) { sh_flag = 0; sh_ncand = 0; sh_count = 0; sh_status = 0; }
+  __syncthreads();
+  // 0. finiteness + 1. axis node: arg-max of s*psi over lim_mask, tie -> smallest n
+  ArgMax am; am.v = -INFINITY; am.n = 0x7fffffff;
+  bool bad = false;
+  for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+    const double v = (double)psi[n];
+    bad |= !isfinite(v);
+    if (D.lim_mask[n]) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
+  }
+  if (bad) atomicOr(&sh_flag, 1);
+  am = block_argmax(am, sh_am);
+  int status = 0;
+  if (sh_flag) status = 2;
+  double Ra = 0, Za = 0, Pa = 0;
+  int ia = -1, ja = -1;
+  if (status == 0) {
+    ja = am.n / nr; ia = am.n - ja * nr;
+    const Fit f = quad_fit(psi + am.n, nr);
+    if (!(f.det > 0.0) || fmax(fabs(f.xs), fabs(f.ys)) > 1.0) status = 1;
+    Ra = D.rmin + (ia + f.xs) * D.dr; Za = D.zmin + (ja + f.ys) * D.dz; Pa = f.ps;
+  }
+  // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
+  if (status == 0) {
+    for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+      if (!D.xpt_mask[n]) continue;
+      const Fit f = quad_fit(psi + n, nr);
+      if (f.det < 0.0 && fabs(f.xs) <= 0.5 && fabs(f.ys) <= 0.5 && sg * f.ps < sg * Pa) {
+        const int q = atomicAdd(&sh_ncand, 1);
+        if (q < PTEFIT_MAX_CAND) {
+          const int j = n / nr, i = n - j * nr;
+          cR[q] = D.rmin + (i + f.xs) * D.dr; cZ[q] = D.zmin + (j + f.ys) * D.dz; cP[q] = f.ps; cN[q] = n;
+        }
+      }
+    }
+  }
+  __syncthreads();
+  const int ncand = sh_ncand;
+  if (status == 0 && ncand > PTEFIT_MAX_CAND) status = 4;
+  // 3. limiter vertices: bilinear flux, valid iff not behind any candidate as seen from the axis
+  ArgMax lm; lm.v = -INFINITY; lm.n = 0x7fffffff;
+  if (status == 0) {
+    for (int v = threadIdx.x; v < D.nlim; v += SEARCH_THREADS) {
+      const double lr = D.lim_r[v], lz = D.lim_z[v];
+      const double fi = (lr - D.rmin) / D.dr, fj = (lz - D.zmin) / D.dz;
+      int i0 = (int)floor(fi), j0 = (int)floor(fj);
+      i0 = max(0, min(i0, nr - 2)); j0 = max(0, min(j0, D.nz - 2));
+      const double tx = fi - i0, ty = fj - j0;
+      const T *p = psi + j0 * nr + i0;
+      const double pv = (1.0 - ty) * ((1.0 - tx) * (double)p[0] + tx * (double)p[1]) +
+                        ty * ((1.0 - tx) * (double)p[nr] + tx * (double)p[nr + 1]);
+      bool valid = true;
+      for (int c = 0; c < ncand; ++c)
+        valid &= ((lr - cR[c]) * (Ra - cR[c]) + (lz - cZ[c]) * (Za - cZ[c])) >= 0.0;
+      if (valid) { ArgMax c; c.v = sg * pv; c.n = v; lm = better(lm, c); }
+    }
+  }
+  lm = block_argmax(lm, sh_am);
+  // 4. boundary flux
+  double Pb = 0.0;
+  if (status == 0) {
+    ArgMax bx; bx.v = -INFINITY; bx.n = 0x7fffffff;
+    int qbest = -1;
+    for (int c = 0; c < ncand; ++c) {
+      ArgMax t; t.v = sg * cP[c]; t.n = cN[c];
+      if (t.v > bx.v || (t.v == bx.v && t.n < bx.n)) { bx = t; qbest = c; }
+    }
+    const bool xwins = bx.v > lm.v;
+    const double spb = xwins ? bx.v : lm.v;
+    if (!isfinite(spb)) status = 1;
+    Pb = sg * spb;
+    if (threadIdx.x == 0) {
+      so.axis_i = ia; so.axis_j = ja; so.axis_r = Ra; so.axis_z = Za; so.axis_psi = Pa;
+      so.n_cand = ncand; so.limited = xwins ? 0 : 1; so.psi_b = Pb;
+      if (qbest >= 0) {
+        so.xpt_j = cN[qbest] / nr; so.xpt_i = cN[qbest] - so.xpt_j * nr;
+        so.xpt_r = cR[qbest]; so.xpt_z = cZ[qbest]; so.xpt_psi = cP[qbest];
+      } else {
+        so.xpt_i = so.xpt_j = -1; so.xpt_r = so.xpt_z = so.xpt_psi = nan("");
+      }
+    }
+    if (Pb == Pa) status = 1;
+  }
+  // 5./6. plasma region and normalised flux
+  int cnt = 0;
+  if (status == 0) {
+    const double inv = 1.0 / (Pb - Pa);
+    for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+      T out = T(-1);
+      if (D.lim_mask[n]) {
+        const double v = (double)psi[n];
+        if (sg * (v - Pb) > 0.0) {
+          const int j = n / nr, i = n - j * nr;
+          const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
+          bool in = true;
+          for (int c = 0; c < ncand; ++c)
+            in &= ((R - cR[c]) * (Ra - cR[c]) + (Z - cZ[c]) * (Za - cZ[c])) > 0.0;
+          if (in) { out = T(fmin(fmax((v - Pa) * inv, 0.0), 1.0)); ++cnt; }
+        }
+      }
+      xn[n] = out;
+    }
+  }
+  if (cnt) atomicAdd(&sh_count, cnt);
+  __syncthreads();
+  if (status == 0 && sh_count == 0) status = 1;
+  if (threadIdx.x == 0) {
+    if (D.status[s] == 0) {
+      if (status == 0 || status == 4) D.so[s] = so;
+      if (status == 1 || status == 2) { SearchOut z = {}; z.axis_i = ia; z.axis_j = ja; z.xpt_i = z.xpt_j = -1; D.so[s] = z; }
+      D.status[s] = status;
+    }
+  }
+}
+
+// Copy the per-slice search results and fit outputs to the caller's arrays.  grid ceil(B/128).
+template <typename T>
+__global__ void k_export(Dev<T> D, int B, T *coeffs, int *axis_ij, T *axis_rzpsi, int *xpt_ij,
+                         T *xpt_rzpsi, T *psi_bnd, int *limited, T *chi2, int *status) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= B) return;
+  const SearchOut o = D.so[s];
+  if (coeffs) for (int l = 0; l < D.nt; ++l) coeffs[(size_t)s * D.nt + l] = T(D.X[(size_t)s * D.nt + l]);
+  if (axis_ij) { axis_ij[2 * s] = o.axis_i; axis_ij[2 * s + 1] = o.axis_j; }
+  if (axis_rzpsi) { axis_rzpsi[3 * s] = T(o.axis_r); axis_rzpsi[3 * s + 1] = T(o.axis_z); axis_rzpsi[3 * s + 2] = T(o.axis_psi); }
+  if (xpt_ij) { xpt_ij[2 * s] = o.xpt_i; xpt_ij[2 * s + 1] = o.xpt_j; }
+  if (xpt_rzpsi) { xpt_rzpsi[3 * s] = T(o.xpt_r); xpt_rzpsi[3 * s + 1] = T(o.xpt_z); xpt_rzpsi[3 * s + 2] = T(o.xpt_psi); }
+  if (psi_bnd) psi_bnd[s] = T(o.psi_b);
+  if (limited) limited[s] = o.limited;
+  if (chi2) chi2[s] = T(D.chi2[s]);
+  if (status) status[s] = D.status[s];
+}
+
+}  // namespace ptefit
