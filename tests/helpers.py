@@ -1,0 +1,79 @@
+"""Shared helpers of the parity tests: input rounding, oracle runs, comparison metrics."""
+import functools
+
+import numpy as np
+
+import synth
+from oracle.picard import Device, reconstruct
+
+PSI_TOL = {"fp32": 1e-5, "fp64": 1e-10}     # north_star: max relative error of psi
+COEF_TOL = 1e-4                              # north_star: basis coefficients, relative
+
+
+def round_inputs(dev, sl, precision):
+    """FP32 mode: the oracle consumes the same inputs the GPU sees (tables, sigma, b, I_C rounded
+    to nearest FP32 and promoted back to FP64).  Returns (dev', b, ic) as float64."""
+    if precision == "fp64":
+        return dev, sl["b"], sl["ic"]
+    r32 = lambda a: np.asarray(a, np.float32).astype(np.float64)
+    d2 = dict(dev)
+    d2["tables"] = {k: r32(v) for k, v in dev["tables"].items()}
+    d2["geom"] = dict(dev["geom"])
+    # sigma stays FP64 in the library (inv_sigma is a double table)
+    return d2, r32(sl["b"]), r32(sl["ic"])
+
+
+@functools.lru_cache(maxsize=4)
+def cached_case(name, n_slices, first=0):
+    dev = synth.make_device(name)
+    sl = synth.make_slices(dev, n_slices, first=first)
+    return dev, sl
+
+
+def oracle_device(dev):
+    return Device(dev["grid"], dev["geom"], dev["tables"], dev["basis"])
+
+
+def psi_rel_err(psi_gpu, psi_or):
+    return float(np.max(np.abs(psi_gpu - psi_or)) / np.max(np.abs(psi_or)))
+
+
+def coef_rel_err(X_gpu, X_or, n_p, n_ff, dz):
+    """Relative to the largest coefficient of the same kind (P' and FF' coefficients differ by
+    ~1e6 in scale); the vertical-shift coefficient (metres) relative to the grid spacing dZ."""
+    e = 0.0
+    e = max(e, np.max(np.abs(X_gpu[:n_p] - X_or[:n_p])) / np.max(np.abs(X_or[:n_p])))
+    e = max(e, np.max(np.abs(X_gpu[n_p:n_p + n_ff] - X_or[n_p:n_p + n_ff])) / np.max(np.abs(X_or[n_p:n_p + n_ff])))
+    if len(X_or) > n_p + n_ff:
+        e = max(e, abs(X_gpu[-1] - X_or[-1]) / dz)
+    return float(e)
+
+
+def check_slice(out, q, ores, dev, precision, strict_index=True):
+    """Compare slice q of the GPU outputs (dict of numpy arrays) with one oracle result."""
+    b = dev["basis"]
+    dz = (dev["grid"]["zmax"] - dev["grid"]["zmin"]) / (dev["grid"]["nz"] - 1)
+    dr = (dev["grid"]["rmax"] - dev["grid"]["rmin"]) / (dev["grid"]["nr"] - 1)
+    assert int(out["status"][q]) == ores["status"], (q, out["status"][q], ores["status"])
+    if ores["status"] != 0:
+        return dict(psi=0.0, coef=0.0, index_ok=True)
+    sr = ores["srch"]
+    epsi = psi_rel_err(out["psi"][q], ores["psi"])
+    ecoef = coef_rel_err(out["coeffs"][q].astype(np.float64), ores["X"], b["n_p"], b["n_ff"], dz)
+    assert epsi <= PSI_TOL[precision], (q, "psi", epsi)
+    assert ecoef <= COEF_TOL, (q, "coef", ecoef)
+    scale = abs(sr["axis"][4] - sr["psi_b"])
+    tol = 1e-4 if precision == "fp32" else 1e-9
+    idx_ok = (tuple(out["axis_ij"][q]) == (sr["axis"][0], sr["axis"][1])
+              and tuple(out["xpt_ij"][q]) == (sr["xpt"][0], sr["xpt"][1]))
+    if strict_index or (sr["axis_margin"] > 1e-4 and not (sr["xpt_margin"] < 1e-4)):
+        assert idx_ok, (q, out["axis_ij"][q], sr["axis"][:2], out["xpt_ij"][q], sr["xpt"][:2], sr["axis_margin"], sr["xpt_margin"])
+    # what is unique regardless of near ties: refined positions and fluxes
+    assert abs(out["axis_rzpsi"][q][0] - sr["axis"][2]) <= tol * dr * 10 + 1e-4 * dr
+    assert abs(out["axis_rzpsi"][q][1] - sr["axis"][3]) <= tol * dz * 10 + 1e-4 * dz
+    assert abs(out["axis_rzpsi"][q][2] - sr["axis"][4]) <= 10 * PSI_TOL[precision] * scale + PSI_TOL[precision] * abs(sr["axis"][4])
+    assert abs(out["psi_bnd"][q] - sr["psi_b"]) <= 10 * PSI_TOL[precision] * scale + PSI_TOL[precision] * abs(sr["psi_b"])
+    if idx_ok:
+        assert int(out["limited"][q]) == sr["limited"]
+    assert abs(out["chi2"][q] / ores["chi2"] - 1) <= (1e-3 if precision == "fp32" else 1e-8)
+    return dict(psi=epsi, coef=ecoef, index_ok=idx_ok)
