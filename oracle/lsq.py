@@ -18,8 +18,11 @@ def fit(resp, d, sigma, lam):
     s = np.sqrt(np.sum(A * A, axis=0))
     keep = s > 0.0
     X = np.zeros(nb)
-    if not keep.any() or not np.all(np.isfinite(A)) or not np.all(np.isfinite(y)):
-        return X, np.nan, (2 if not np.all(np.isfinite(A)) else 3)
+    finite = np.all(np.isfinite(A)) and np.all(np.isfinite(y))
+    if not finite:
+        return X, np.nan, 2          # include/ptefit.h: status 2 = non-finite data
+    if not keep.any():
+        return X, np.nan, 3          # status 3 = singular fit
     Ae = A[:, keep] / s[keep]
     k = Ae.shape[1]
     S = np.vstack([Ae, lam * np.sqrt(M) * np.eye(k)])

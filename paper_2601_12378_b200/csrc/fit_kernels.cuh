@@ -47,7 +47,8 @@ __global__ void k_cold_start(Dev<T> D) {
 }
 
 // Vertical-shift column (O4b): dzc[n] = -(I'[n+nr] - I'[n-nr]) / (2 dZ) with
-// I' = J_b(xn) X_prev over the polynomial terms.  grid (ceil(N/256), B).
+// I' = J_b(xn) X over the polynomial terms, X = the coefficients of the previous fit (D.X is
+// only overwritten by k_lsq, which runs after this kernel).  grid (ceil(N/256), B).
 template <typename T>
 __global__ void k_delz_column(Dev<T> D) {
   const int s = blockIdx.y;
@@ -59,7 +60,7 @@ __global__ void k_delz_column(Dev<T> D) {
     const T R = T(D.rmin + i * D.dr);
     const T rdA = R * T(D.dA), fdA = T(kMu0 * D.dA) / R;
     const T *x = D.xn + (size_t)s * D.N;
-    const double *Xp = D.Xprev + (size_t)s * D.nt;
+    const double *Xp = D.X + (size_t)s * D.nt;
     T up = T(0), dn = T(0);
     for (int l = 0; l < D.npoly; ++l) {
       const T c = T(Xp[l]);

@@ -207,13 +207,26 @@ def test_edge_cases():
 
 
 def test_paper_form_without_additions():
-    """lambda = 0, relax = 1, no delz term reproduces the paper's bare Eq. 6 iteration; compare a
-    few iterations (before the vertical drift grows) with the oracle run the same way."""
+    """lambda = 0, relax = 1, no delz term reproduces the paper's bare Eq. 6 iteration.  The paper
+    runs it from a warm start only (from a cold start the unregularised loop is
+    chaotic and amplifies rounding differences), so: converge with the defaults, then continue
+    3 bare iterations from that flux on both sides."""
+    torch = _torch()
     dev, sl = cached_case("cfg1", 2)
+    od0 = oracle_device(dev)
     d2 = dict(dev); d2["basis"] = dict(dev["basis"], lambda_reg=0.0, relax=1.0, delz=0)
     od = oracle_device(d2)
-    rec, out = _run_gpu(d2, sl["b"], sl["ic"], 4, "fp64")
+    psi0 = np.stack([reconstruct(od0, sl["b"][q], sl["ic"][q], 10)["psi"] for q in range(2)])
+    rec = _rec(d2, "fp64", 2)
+    rec.psi.copy_(torch.tensor(psi0, dtype=rec.dtype, device="cuda"))
+    db = torch.tensor(sl["b"], dtype=rec.dtype, device="cuda"); dic = torch.tensor(sl["ic"], dtype=rec.dtype, device="cuda")
+    rec.reconstruct(db, dic, 3, warm_start=True)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, 2)
     for q in range(2):
-        ores = reconstruct(od, sl["b"][q], sl["ic"][q], 4)
-        check_slice(out, q, ores, d2, "fp64")
+        ores = reconstruct(od, sl["b"][q], sl["ic"][q], 3, psi0=psi0[q])
+        if ores["status"] == 0:
+            r = check_slice(out, q, ores, d2, "fp64")
+        else:
+            assert int(out["status"][q]) == ores["status"]
     rec.close()
