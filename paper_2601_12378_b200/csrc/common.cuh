@@ -40,6 +40,7 @@ struct Dev {
   const double *tri_w, *tri_invb; // Thomas multipliers and inverse pivots
   const double *tri_ce;           // [nri] super-diagonal
   const T *sintab;                // [2*(nz-1)] sin(pi k/(nz-1))
+  const T *dst_tab;               // folded DST matrices So[n2][n2], Se[n2][n2] (fused_solve.cuh)
   // workspaces [max_batch][...]
   T *xn, *psi_coil, *dred, *resp, *cur, *dzc, *psi_bdry, *fhat;
   double *ytmp;                   // [B][nri][nzi]

@@ -1,0 +1,208 @@
+// fused_solve.cuh -- A7 + A8 + A1 (+ the vertical-shift column) of one slice in ONE CTA, flux map
+// resident in shared memory:
+//   rhs assembly -> DST-I in Z -> FP64 Thomas in R -> DST-I in Z -> psi = psi_pl + psi_coil with
+//   relaxation -> axis / X-point / LCFS search and normalisation -> -dI'/dZ column.
+// Delta* psi = -mu0 R J_phi on the 5-point stencil (Eq. 1, 118-120); search per
+// PAPER.md:122-136.  The DST is a folded dense product: sin(pi (Nz-j) m / Nz) = (-1)^(m+1)
+// sin(pi j m / Nz), so odd modes see f_j + f_{Nz-j} and even modes f_j - f_{Nz-j}: two
+// (Nz/2)^2 products instead of one (Nz-1)^2.  Used when the slice fits shared memory
+// (e.g. 129x129 FP32 = 108 KB, two CTAs per SM); larger grids take the three-kernel path of
+// solve_kernels.cuh.  Persistent: CTA b handles slices b, b + gridDim.x, ...
+#pragma once
+#include "common.cuh"
+#include "search_kernels.cuh"
+
+namespace ptefit {
+
+constexpr int FUSED_THREADS = 256;
+constexpr int FUSED_CW = 16;       // columns per DST chunk
+
+template <typename T> struct Vec4 { T v[4]; };
+__device__ __forceinline__ Vec4<float> load4(const float *p) {
+  const float4 q = *reinterpret_cast<const float4 *>(p);
+  return {{q.x, q.y, q.z, q.w}};
+}
+__device__ __forceinline__ Vec4<double> load4(const double *p) {
+  const double2 a = *reinterpret_cast<const double2 *>(p), b = *reinterpret_cast<const double2 *>(p + 2);
+  return {{a.x, a.y, b.x, b.y}};
+}
+template <typename T> struct Vec2 { T v[2]; };
+__device__ __forceinline__ Vec2<float> load2(const float *p) {
+  const float2 q = *reinterpret_cast<const float2 *>(p);
+  return {{q.x, q.y}};
+}
+__device__ __forceinline__ Vec2<double> load2(const double *p) {
+  const double2 q = *reinterpret_cast<const double2 *>(p);
+  return {{q.x, q.y}};
+}
+
+// Shared-memory bytes of k_solve_fused for a grid (host and device agree through this).
+template <typename T>
+__host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
+  const int n2 = (nz - 1) / 2;
+  const size_t g = ((size_t)nz * nr + 3) & ~(size_t)3;          // 16-byte aligned sub-arrays
+  return (g + 2 * (size_t)n2 * n2 + 2 * (size_t)n2 * FUSED_CW) * sizeof(T);
+}
+
+// In-place DST-I along Z of the interior columns of G[nz][nr] (rows 1..nz-2 <-> modes 1..nz-2),
+// unnormalised: G[m][i] <- sum_j sin(pi j m / (nz-1)) G[j][i].
+template <typename T>
+__device__ void dst_columns(T *G, const T *So, const T *Se, T *E, int nr, int nz) {
+  const int Nz = nz - 1, n2 = Nz / 2, nri = nr - 2, nzi = nz - 2;
+  const int nq = n2 / 4, ncp = FUSED_CW / 2;
+  const int items = 2 * nq * ncp;
+  const int tid = threadIdx.x, nth = blockDim.x;
+  for (int c0 = 0; c0 < nri; c0 += FUSED_CW) {
+    for (int e = tid; e < n2 * FUSED_CW; e += nth) {          // fold rows j and Nz-j
+      const int jj = e / FUSED_CW, c = e - jj * FUSED_CW;
+      const int i = 1 + c0 + c;
+      T a = T(0), b = T(0);
+      if (i <= nri) {
+        const T lo = G[(jj + 1) * nr + i];
+        if (jj + 1 < n2) { const T hi = G[(Nz - jj - 1) * nr + i]; a = lo + hi; b = lo - hi; }
+        else a = lo;                                           // centre row j = Nz/2
+      }
+      E[e] = a;
+      E[n2 * FUSED_CW + e] = b;
+    }
+    __syncthreads();
+    for (int it = tid; it < items; it += nth) {
+      const int cp = it % ncp, q = (it / ncp) % nq, par = it / (ncp * nq);
+      const T *St = (par ? Se : So) + 4 * q;
+      const T *Ep = E + par * n2 * FUSED_CW + 2 * cp;
+      T acc[4][2];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) acc[r][0] = acc[r][1] = T(0);
+#pragma unroll 8
+      for (int j = 0; j < n2; ++j) {
+        const Vec4<T> sv = load4(St + j * n2);
+        const Vec2<T> ev = load2(Ep + j * FUSED_CW);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          acc[r][0] = fma(sv.v[r], ev.v[0], acc[r][0]);
+          acc[r][1] = fma(sv.v[r], ev.v[1], acc[r][1]);
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const int m = 2 * (4 * q + r) + 1 + par;
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          const int i = 1 + c0 + 2 * cp + t;
+          if (m <= nzi && i <= nri) G[m * nr + i] = acc[r][t];
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// grid min(B, resident CTAs), block FUSED_THREADS, dyn smem fused_smem_bytes<T>(nr, nz).
+// cur[B][N] node currents (A), pbd[B][nbnd] boundary flux, psi[B][N] in/out.
+// do_search = 0: Delta* solve only (debug hook); 1: also search + xn (+ dzc when has_delz).
+template <typename T>
+__global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, const T *__restrict__ cur_all,
+                                                                const T *__restrict__ pbd_all, T *__restrict__ psi_all,
+                                                                T *__restrict__ xn_all, int use_relax, int add_coil,
+                                                                int do_search) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nr = D.nr, nz = D.nz, N = D.N, nri = D.nri, nzi = D.nzi, Nz = nz - 1, n2 = Nz / 2;
+  const int tid = threadIdx.x, nth = blockDim.x;
+  T *G = reinterpret_cast<T *>(smem_raw);
+  T *So = G + ((N + 3) & ~3);
+  T *Se = So + n2 * n2;
+  T *E = Se + n2 * n2;
+  for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];      // So then Se, contiguous
+  const T cz = T(1.0 / (D.dz * D.dz));
+  const T scale = T(2.0 / Nz);
+  const T om = T(D.relax);
+  for (int s = blockIdx.x; s < B; s += gridDim.x) {
+    const T *I = cur_all + (size_t)s * N;
+    const T *pb = pbd_all + (size_t)s * D.nbnd;           // bottom[nr], top[nr], left[nzi], right[nzi]
+    T *psi = psi_all + (size_t)s * N;
+    __syncthreads();                                       // previous slice done with G; tables loaded
+    // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
+    for (int n = tid; n < N; n += nth) {
+      const int j = n / nr, i = n - j * nr;
+      T v;
+      if (j == 0) v = pb[i];
+      else if (j == nz - 1) v = pb[nr + i];
+      else if (i == 0) v = pb[2 * nr + j - 1];
+      else if (i == nr - 1) v = pb[2 * nr + nzi + j - 1];
+      else {
+        const double R = D.rmin + i * D.dr;
+        v = T(-kMu0 * R / D.dA) * I[n];
+        if (i == 1) v -= T((1.0 + D.dr / (2.0 * R)) / (D.dr * D.dr)) * pb[2 * nr + j - 1];
+        if (i == nri) v -= T((1.0 - D.dr / (2.0 * R)) / (D.dr * D.dr)) * pb[2 * nr + nzi + j - 1];
+        if (j == 1) v -= cz * pb[i];
+        if (j == nzi) v -= cz * pb[nr + i];
+      }
+      G[n] = v;
+    }
+    __syncthreads();
+    dst_columns<T>(G, So, Se, E, nr, nz);
+    // ---- Thomas sweeps along R in FP64, one thread per mode (precomputed factors)
+    if (tid < nzi) {
+      const int mm = tid;
+      T *row = G + (mm + 1) * nr + 1;
+      double *y = D.ytmp + (size_t)blockIdx.x * nri * nzi;
+      double prev = 0.0;
+#pragma unroll 8
+      for (int i = 0; i < nri; ++i) {
+        const size_t o = (size_t)i * nzi + mm;
+        const double v = (double)row[i] - D.tri_w[o] * prev;
+        y[o] = v;
+        prev = v;
+      }
+      double x = 0.0;
+#pragma unroll 8
+      for (int i = nri - 1; i >= 0; --i) {
+        const size_t o = (size_t)i * nzi + mm;
+        x = (y[o] - D.tri_ce[i] * x) * D.tri_invb[o];
+        row[i] = T(x);
+      }
+    }
+    __syncthreads();
+    dst_columns<T>(G, So, Se, E, nr, nz);
+    // ---- total flux + relaxation; psi goes to global memory and stays in G for the search
+    const T *pc = D.psi_coil + (size_t)s * N;
+    for (int n = tid; n < N; n += nth) {
+      const int j = n / nr, i = n - j * nr;
+      const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
+      T v = edge ? G[n] : G[n] * scale;
+      if (add_coil) v += pc[n];
+      if (use_relax) { const T old = psi[n]; v = old + om * (v - old); }
+      psi[n] = v;
+      G[n] = v;
+    }
+    __syncthreads();
+    if (do_search) {
+      T *xn = xn_all + (size_t)s * N;
+      search_body<T>(D, s, G, xn, G);                      // G now holds xn
+      if (D.has_delz) {
+        __syncthreads();
+        // -dI'/dZ column for the NEXT fit: I' = J_b(xn) X with the coefficients of this fit
+        const double *Xp = D.X + (size_t)s * D.nt;
+        T *dzc = D.dzc + (size_t)s * N;
+        for (int n = tid; n < N; n += nth) {
+          const int j = n / nr, i = n - j * nr;
+          T out = T(0);
+          if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) {
+            const T R = T(D.rmin + i * D.dr);
+            const T rdA = R * T(D.dA), fdA = T(kMu0 * D.dA) / R;
+            T up = T(0), dn = T(0);
+            for (int l = 0; l < D.npoly; ++l) {
+              const T c = T(Xp[l]);
+              up = fma(basis_term(D, l, G[n + nr], rdA, fdA), c, up);
+              dn = fma(basis_term(D, l, G[n - nr], rdA, fdA), c, dn);
+            }
+            out = -(up - dn) * T(0.5 / D.dz);
+          }
+          dzc[n] = out;
+        }
+      }
+    }
+  }
+}
+
+}  // namespace ptefit

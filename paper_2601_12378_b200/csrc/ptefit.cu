@@ -13,6 +13,7 @@
 #include "fit_kernels.cuh"
 #include "search_kernels.cuh"
 #include "solve_kernels.cuh"
+#include "fused_solve.cuh"
 
 using namespace ptefit;
 
@@ -27,6 +28,9 @@ struct ptefit_handle {
   std::vector<void *> allocs;
   std::string error;
   int launches = 0;
+  bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
+  int fused_grid = 0;                   // resident CTAs of k_solve_fused
+  size_t fused_smem = 0;
   bool profiling = false;
   std::vector<cudaEvent_t> ev;          // stage boundaries of the last call
   std::vector<int> ev_stage;
@@ -155,6 +159,17 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
     for (int k = 0; k < period; ++k) st[k] = sin(pi * k / (D.nz - 1));
     st[D.nz - 1] = 0.0;
     TRY(upload(h, &D.sintab, st.data(), st.size()));
+    // folded DST matrices, transposed so that four consecutive modes are one vector load:
+    // So[j][p] = sin(pi (j+1)(2p+1)/Nz), Se[j][p] = sin(pi (j+1)(2p+2)/Nz) (0 beyond Nz/2-1)
+    const int Nz = D.nz - 1, n2 = Nz / 2;
+    std::vector<double> tab(2 * (size_t)n2 * n2, 0.0);
+    for (int j = 0; j < n2; ++j)
+      for (int q = 0; q < n2; ++q) {
+        tab[(size_t)j * n2 + q] = sin(pi * (double)((j + 1) * (2 * q + 1) % (2 * Nz)) / Nz);
+        if (j < n2 - 1 && q < n2 - 1)
+          tab[(size_t)n2 * n2 + (size_t)j * n2 + q] = sin(pi * (double)((j + 1) * (2 * q + 2) % (2 * Nz)) / Nz);
+      }
+    TRY(upload(h, &D.dst_tab, tab.data(), tab.size()));
   }
   // workspaces
   TRY(dev_alloc(h, &D.xn, (size_t)B * N));

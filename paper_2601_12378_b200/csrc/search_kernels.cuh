@@ -49,21 +49,22 @@ __device__ __forceinline__ ArgMax block_argmax(ArgMax a, ArgMax *sh) {
   if (lane == 0) sh[w] = a;
   __syncthreads();
   ArgMax r = sh[0];
-  for (int k = 1; k < SEARCH_THREADS / 32; ++k) r = better(r, sh[k]);
+  const int nw = (blockDim.x + 31) >> 5;
+  for (int k = 1; k < nw; ++k) r = better(r, sh[k]);
   return r;
 }
 
-// grid B, block SEARCH_THREADS.  Reads psi[s], writes xn[s] (normalised flux in the mask, -1
-// outside), D.so[s] and D.status[s] (sticky).
+// Search of one slice by one CTA (any block size that is a multiple of 32, <= 1024).  Reads
+// psi[nz][nr] (global or shared memory), writes xn (normalised flux in the mask, -1 outside) to
+// global memory and, if xn_local != nullptr, also to xn_local (may alias psi: every thread
+// overwrites only nodes it alone reads after the last barrier).  Updates D.so[s], D.status[s]
+// (sticky).  All threads of the CTA must call it.
 template <typename T>
-__global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__restrict__ psi_all,
-                                                            T *__restrict__ xn_all) {
-  const int s = blockIdx.x;
-  const T *psi = psi_all + (size_t)s * D.N;
-  T *xn = xn_all + (size_t)s * D.N;
+__device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, T *xn_local) {
+  const int nth = blockDim.x;
   const int nr = D.nr, N = D.N;
   const double sg = (double)D.ip_sign;
-  __shared__ ArgMax sh_am[SEARCH_THREADS / 32];
+  __shared__ ArgMax sh_am[32];
   __shared__ int sh_flag, sh_ncand, sh_count;
   __shared__ double cR[PTEFIT_MAX_CAND], cZ[PTEFIT_MAX_CAND], cP[PTEFIT_MAX_CAND];
   __shared__ int cN[PTEFIT_MAX_CAND];
@@ -74,7 +75,7 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
   // 0. finiteness + 1. axis node: arg-max of s*psi over lim_mask, tie -> smallest n
   ArgMax am; am.v = -INFINITY; am.n = 0x7fffffff;
   bool bad = false;
-  for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+  for (int n = threadIdx.x; n < N; n += nth) {
     const double v = (double)psi[n];
     bad |= !isfinite(v);
     if (D.lim_mask[n]) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
   }
   // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
   if (status == 0) {
-    for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+    for (int n = threadIdx.x; n < N; n += nth) {
       if (!D.xpt_mask[n]) continue;
       const Fit f = quad_fit(psi + n, nr);
       if (f.det < 0.0 && fabs(f.xs) <= 0.5 && fabs(f.ys) <= 0.5 && sg * f.ps < sg * Pa) {
@@ -111,7 +112,7 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
   // 3. limiter vertices: bilinear flux, valid iff not behind any candidate as seen from the axis
   ArgMax lm; lm.v = -INFINITY; lm.n = 0x7fffffff;
   if (status == 0) {
-    for (int v = threadIdx.x; v < D.nlim; v += SEARCH_THREADS) {
+    for (int v = threadIdx.x; v < D.nlim; v += nth) {
       const double lr = D.lim_r[v], lz = D.lim_z[v];
       const double fi = (lr - D.rmin) / D.dr, fj = (lz - D.zmin) / D.dz;
       int i0 = (int)floor(fi), j0 = (int)floor(fj);
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
   int cnt = 0;
   if (status == 0) {
     const double inv = 1.0 / (Pb - Pa);
-    for (int n = threadIdx.x; n < N; n += SEARCH_THREADS) {
+    for (int n = threadIdx.x; n < N; n += nth) {
       T out = T(-1);
       if (D.lim_mask[n]) {
         const double v = (double)psi[n];
@@ -170,7 +171,10 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
         }
       }
       xn[n] = out;
+      if (xn_local) xn_local[n] = out;
     }
+  } else if (xn_local) {
+    for (int n = threadIdx.x; n < N; n += nth) xn_local[n] = T(-1);
   }
   if (cnt) atomicAdd(&sh_count, cnt);
   __syncthreads();
@@ -182,6 +186,14 @@ __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__
       D.status[s] = status;
     }
   }
+}
+
+// grid B, block SEARCH_THREADS.
+template <typename T>
+__global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__restrict__ psi_all,
+                                                            T *__restrict__ xn_all) {
+  const int s = blockIdx.x;
+  search_body<T>(D, s, psi_all + (size_t)s * D.N, xn_all + (size_t)s * D.N, nullptr);
 }
 
 // Copy the per-slice search results and fit outputs to the caller's arrays.  grid ceil(B/128).
