@@ -145,21 +145,40 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
     if (tid < nzi) {
       const int mm = tid;
       T *row = G + (mm + 1) * nr + 1;
-      double *y = D.ytmp + (size_t)blockIdx.x * nri * nzi;
+      double *__restrict__ y = D.ytmp + (size_t)blockIdx.x * nri * nzi + mm;
+      const double *__restrict__ tw = D.tri_w + mm;
+      const double *__restrict__ tb = D.tri_invb + mm;
+      const double *__restrict__ tce = D.tri_ce;
+      constexpr int U = 8;                     // factor loads of U steps are issued before the chain
       double prev = 0.0;
-#pragma unroll 8
-      for (int i = 0; i < nri; ++i) {
-        const size_t o = (size_t)i * nzi + mm;
-        const double v = (double)row[i] - D.tri_w[o] * prev;
-        y[o] = v;
-        prev = v;
+      for (int i0 = 0; i0 < nri; i0 += U) {
+        double w[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) w[u] = (i0 + u < nri) ? __ldg(tw + (size_t)(i0 + u) * nzi) : 0.0;
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+          if (i0 + u < nri) {
+            const double v = (double)row[i0 + u] - w[u] * prev;
+            y[(size_t)(i0 + u) * nzi] = v;
+            prev = v;
+          }
       }
       double x = 0.0;
-#pragma unroll 8
-      for (int i = nri - 1; i >= 0; --i) {
-        const size_t o = (size_t)i * nzi + mm;
-        x = (y[o] - D.tri_ce[i] * x) * D.tri_invb[o];
-        row[i] = T(x);
+      for (int i0 = nri - 1; i0 >= 0; i0 -= U) {
+        double yy[U], ib[U], ce[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int i = i0 - u;
+          yy[u] = i >= 0 ? y[(size_t)i * nzi] : 0.0;
+          ib[u] = i >= 0 ? __ldg(tb + (size_t)i * nzi) : 0.0;
+          ce[u] = i >= 0 ? __ldg(tce + i) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+          if (i0 - u >= 0) {
+            x = (yy[u] - ce[u] * x) * ib[u];
+            row[i0 - u] = T(x);
+          }
       }
     }
     __syncthreads();
