@@ -8,6 +8,8 @@
 #define PTEFIT_MAX_TERMS 12
 #define PTEFIT_MAX_CAND 32
 #define PTEFIT_MAX_LIM 256
+#define PTEFIT_MAX_NR 257
+#define PTEFIT_MAX_DEG 8      /* largest exponent N of a polynomial term */
 
 namespace ptefit {
 

@@ -113,6 +113,19 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
   T *Se = So + n2 * n2;
   T *E = Se + n2 * n2;
   for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];      // So then Se, contiguous
+  // per-column constants (same expressions as the unfused kernels, evaluated once per CTA)
+  __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
+  __shared__ T pcoef[2][PTEFIT_MAX_DEG + 1];                 // I'(x) = rdA P(x) + fdA Q(x)
+  __shared__ T c_edge[2];
+  for (int i = tid; i < nr; i += nth) {
+    const double Rd = D.rmin + i * D.dr;
+    c_rhs[i] = T(-kMu0 * Rd / D.dA);
+    const T R = T(Rd);
+    c_rdA[i] = R * T(D.dA);
+    c_fdA[i] = T(kMu0 * D.dA) / R;
+    if (i == 1) c_edge[0] = T((1.0 + D.dr / (2.0 * Rd)) / (D.dr * D.dr));
+    if (i == nri) c_edge[1] = T((1.0 - D.dr / (2.0 * Rd)) / (D.dr * D.dr));
+  }
   const T cz = T(1.0 / (D.dz * D.dz));
   const T scale = T(2.0 / Nz);
   const T om = T(D.relax);
@@ -122,22 +135,25 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
     T *psi = psi_all + (size_t)s * N;
     __syncthreads();                                       // previous slice done with G; tables loaded
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
-    for (int n = tid; n < N; n += nth) {
-      const int j = n / nr, i = n - j * nr;
-      T v;
-      if (j == 0) v = pb[i];
-      else if (j == nz - 1) v = pb[nr + i];
-      else if (i == 0) v = pb[2 * nr + j - 1];
-      else if (i == nr - 1) v = pb[2 * nr + nzi + j - 1];
-      else {
-        const double R = D.rmin + i * D.dr;
-        v = T(-kMu0 * R / D.dA) * I[n];
-        if (i == 1) v -= T((1.0 + D.dr / (2.0 * R)) / (D.dr * D.dr)) * pb[2 * nr + j - 1];
-        if (i == nri) v -= T((1.0 - D.dr / (2.0 * R)) / (D.dr * D.dr)) * pb[2 * nr + nzi + j - 1];
-        if (j == 1) v -= cz * pb[i];
-        if (j == nzi) v -= cz * pb[nr + i];
+    {
+      int j = tid / nr, i = tid - j * nr;
+      for (int n = tid; n < N; n += nth) {
+        T v;
+        if (j == 0) v = pb[i];
+        else if (j == nz - 1) v = pb[nr + i];
+        else if (i == 0) v = pb[2 * nr + j - 1];
+        else if (i == nr - 1) v = pb[2 * nr + nzi + j - 1];
+        else {
+          v = c_rhs[i] * I[n];
+          if (i == 1) v -= c_edge[0] * pb[2 * nr + j - 1];
+          if (i == nri) v -= c_edge[1] * pb[2 * nr + nzi + j - 1];
+          if (j == 1) v -= cz * pb[i];
+          if (j == nzi) v -= cz * pb[nr + i];
+        }
+        G[n] = v;
+        i += nth;
+        while (i >= nr) { i -= nr; ++j; }
       }
-      G[n] = v;
     }
     __syncthreads();
     dst_columns<T>(G, So, Se, E, nr, nz);
@@ -185,39 +201,60 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
     dst_columns<T>(G, So, Se, E, nr, nz);
     // ---- total flux + relaxation; psi goes to global memory and stays in G for the search
     const T *pc = D.psi_coil + (size_t)s * N;
-    for (int n = tid; n < N; n += nth) {
-      const int j = n / nr, i = n - j * nr;
-      const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
-      T v = edge ? G[n] : G[n] * scale;
-      if (add_coil) v += pc[n];
-      if (use_relax) { const T old = psi[n]; v = old + om * (v - old); }
-      psi[n] = v;
-      G[n] = v;
+    {
+      int j = tid / nr, i = tid - j * nr;
+      for (int n = tid; n < N; n += nth) {
+        const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
+        T v = edge ? G[n] : G[n] * scale;
+        if (add_coil) v += pc[n];
+        if (use_relax) { const T old = psi[n]; v = old + om * (v - old); }
+        psi[n] = v;
+        G[n] = v;
+        i += nth;
+        while (i >= nr) { i -= nr; ++j; }
+      }
     }
     __syncthreads();
     if (do_search) {
       T *xn = xn_all + (size_t)s * N;
       search_body<T>(D, s, G, xn, G);                      // G now holds xn
       if (D.has_delz) {
+        // -dI'/dZ column for the NEXT fit: I' = J_b(xn) X with the coefficients of this fit.
+        // The P'/FF' sums are polynomials in x: collect their coefficients once per slice,
+        // evaluate I' per node by Horner in place of xn, then difference along Z.
+        if (tid < 2 * (PTEFIT_MAX_DEG + 1)) {
+          const int kind = tid / (PTEFIT_MAX_DEG + 1), k = tid - kind * (PTEFIT_MAX_DEG + 1);
+          const double *Xp = D.X + (size_t)s * D.nt;
+          double c = 0.0;
+          for (int l = 0; l < D.npoly; ++l)
+            if (D.terms[l].kind == kind) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+          pcoef[kind][k] = T(c);
+        }
         __syncthreads();
-        // -dI'/dZ column for the NEXT fit: I' = J_b(xn) X with the coefficients of this fit
-        const double *Xp = D.X + (size_t)s * D.nt;
-        T *dzc = D.dzc + (size_t)s * N;
-        for (int n = tid; n < N; n += nth) {
-          const int j = n / nr, i = n - j * nr;
-          T out = T(0);
-          if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) {
-            const T R = T(D.rmin + i * D.dr);
-            const T rdA = R * T(D.dA), fdA = T(kMu0 * D.dA) / R;
-            T up = T(0), dn = T(0);
-            for (int l = 0; l < D.npoly; ++l) {
-              const T c = T(Xp[l]);
-              up = fma(basis_term(D, l, G[n + nr], rdA, fdA), c, up);
-              dn = fma(basis_term(D, l, G[n - nr], rdA, fdA), c, dn);
-            }
-            out = -(up - dn) * T(0.5 / D.dz);
+        {
+          int j = tid / nr, i = tid - j * nr;
+          for (int n = tid; n < N; n += nth) {
+            const T x = G[n];
+            T hp = pcoef[0][PTEFIT_MAX_DEG], hq = pcoef[1][PTEFIT_MAX_DEG];
+#pragma unroll
+            for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fma(hp, x, pcoef[0][k]); hq = fma(hq, x, pcoef[1][k]); }
+            G[n] = (x < T(0)) ? T(0) : fma(c_rdA[i], hp, c_fdA[i] * hq);
+            i += nth;
+            while (i >= nr) { i -= nr; ++j; }
           }
-          dzc[n] = out;
+        }
+        __syncthreads();
+        T *dzc = D.dzc + (size_t)s * N;
+        const T hz = T(0.5 / D.dz);
+        {
+          int j = tid / nr, i = tid - j * nr;
+          for (int n = tid; n < N; n += nth) {
+            T out = T(0);
+            if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) out = -(G[n + nr] - G[n - nr]) * hz;
+            dzc[n] = out;
+            i += nth;
+            while (i >= nr) { i -= nr; ++j; }
+          }
         }
       }
     }

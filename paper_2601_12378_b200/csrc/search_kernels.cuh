@@ -13,23 +13,33 @@ struct Fit { double det, xs, ys, ps; };
 
 // 3x3 least-squares quadratic with the pre-inverted normal equations: integer
 // weight table, index units.  p points at the centre node, ld = nr.
+struct Quad { double cx, cy, cxx, cyy, cxy, c0, det; };
 template <typename T>
-__device__ __forceinline__ Fit quad_fit(const T *__restrict__ p, int ld) {
+__device__ __forceinline__ Quad quad_coef(const T *__restrict__ p, int ld) {
   const double a = p[-ld - 1], b = p[-ld], c = p[-ld + 1];
   const double d = p[-1], e = p[0], f = p[1];
   const double g = p[ld - 1], h = p[ld], k = p[ld + 1];
-  const double cx = ((c + f + k) - (a + d + g)) * (1.0 / 6.0);
-  const double cy = ((g + h + k) - (a + b + c)) * (1.0 / 6.0);
-  const double cxx = ((a + d + g) - 2.0 * (b + e + h) + (c + f + k)) * (1.0 / 6.0);
-  const double cyy = ((a + b + c) - 2.0 * (d + e + f) + (g + h + k)) * (1.0 / 6.0);
-  const double cxy = (k + a - g - c) * 0.25;
-  const double c0 = (5.0 * e + 2.0 * (b + d + f + h) - (a + c + g + k)) * (1.0 / 9.0);
+  Quad q;
+  q.cx = ((c + f + k) - (a + d + g)) * (1.0 / 6.0);
+  q.cy = ((g + h + k) - (a + b + c)) * (1.0 / 6.0);
+  q.cxx = ((a + d + g) - 2.0 * (b + e + h) + (c + f + k)) * (1.0 / 6.0);
+  q.cyy = ((a + b + c) - 2.0 * (d + e + f) + (g + h + k)) * (1.0 / 6.0);
+  q.cxy = (k + a - g - c) * 0.25;
+  q.c0 = (5.0 * e + 2.0 * (b + d + f + h) - (a + c + g + k)) * (1.0 / 9.0);
+  q.det = 4.0 * q.cxx * q.cyy - q.cxy * q.cxy;
+  return q;
+}
+__device__ __forceinline__ Fit quad_finish(const Quad &q) {
   Fit o;
-  o.det = 4.0 * cxx * cyy - cxy * cxy;
-  o.xs = -(2.0 * cyy * cx - cxy * cy) / o.det;
-  o.ys = -(2.0 * cxx * cy - cxy * cx) / o.det;
-  o.ps = c0 + 0.5 * (cx * o.xs + cy * o.ys);
+  o.det = q.det;
+  o.xs = -(2.0 * q.cyy * q.cx - q.cxy * q.cy) / q.det;
+  o.ys = -(2.0 * q.cxx * q.cy - q.cxy * q.cx) / q.det;
+  o.ps = q.c0 + 0.5 * (q.cx * o.xs + q.cy * o.ys);
   return o;
+}
+template <typename T>
+__device__ __forceinline__ Fit quad_fit(const T *__restrict__ p, int ld) {
+  return quad_finish(quad_coef<T>(p, ld));
 }
 
 struct ArgMax { double v; int n; };
@@ -96,7 +106,9 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   if (status == 0) {
     for (int n = threadIdx.x; n < N; n += nth) {
       if (!D.xpt_mask[n]) continue;
-      const Fit f = quad_fit(psi + n, nr);
+      const Quad qc = quad_coef(psi + n, nr);
+      if (!(qc.det < 0.0)) continue;                  // the divisions only for saddle-like nodes
+      const Fit f = quad_finish(qc);
       if (f.det < 0.0 && fabs(f.xs) <= 0.5 && fabs(f.ys) <= 0.5 && sg * f.ps < sg * Pa) {
         const int q = atomicAdd(&sh_ncand, 1);
         if (q < PTEFIT_MAX_CAND) {
