@@ -11,7 +11,7 @@ LIB_PATH = os.path.join(HERE, "libptefit.so")
 EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
-    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms",
+    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_debug_phase_clocks",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
@@ -86,6 +86,8 @@ def load_library():
         lib.ptefit_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.ptefit_get_stage_ms.restype = C.c_int
         lib.ptefit_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        lib.ptefit_debug_phase_clocks.restype = C.c_int
+        lib.ptefit_debug_phase_clocks.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong)]
         _lib = lib
     return _lib
 
@@ -242,6 +244,11 @@ class Reconstructor:
         out = (C.c_float * 6)()
         self._call(self.lib.ptefit_get_stage_ms, out)
         return dict(zip(("setup", "response", "lsq", "boundary", "solve", "search"), list(out)))
+
+    def phase_clocks(self, on=True, read=False):
+        out = (C.c_longlong * 8)() if read else None
+        self._call(self.lib.ptefit_debug_phase_clocks, int(on), out)
+        return list(out) if read else None
 
     def close(self):
         if self.h is not None:

@@ -37,6 +37,7 @@ struct Dev {
   const T *gp, *gc, *gb, *ggc;
   const double *inv_sigma;        // [M]
   const uint8_t *lim_mask, *xpt_mask;
+  const unsigned *lim_bits, *xpt_bits;   // the same masks bit-packed: bit (n & 31) of word n >> 5
   const double *lim_r, *lim_z;    // [nlim]
   // Delta* solve factors: [nri][nzi] (i-major so that threads over m coalesce)
   const double *tri_w, *tri_invb; // Thomas multipliers and inverse pivots
@@ -50,6 +51,7 @@ struct Dev {
   double *chi2;                   // [B]
   SearchOut *so;                  // [B]
   int *status;                    // [B]
+  long long *phase_clk;           // [8] optional in-kernel phase timers (ptefit_debug_phase_clocks), else nullptr
 };
 
 __device__ __forceinline__ double warp_sum(double v) {

@@ -41,7 +41,11 @@ template <typename T>
 __host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
   const int n2 = (nz - 1) / 2;
   const size_t g = ((size_t)nz * nr + 3) & ~(size_t)3;          // 16-byte aligned sub-arrays
-  return (g + 2 * (size_t)n2 * n2 + 2 * (size_t)n2 * FUSED_CW) * sizeof(T);
+  size_t e = 2 * (size_t)n2 * FUSED_CW * sizeof(T);               // fold buffer, reused for the bit masks
+  const size_t mb = 2 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);
+  if (mb > e) e = mb;
+  e = (e + 15) & ~(size_t)15;
+  return (g + 2 * (size_t)n2 * n2) * sizeof(T) + e;
 }
 
 // In-place DST-I along Z of the interior columns of G[nz][nr] (rows 1..nz-2 <-> modes 1..nz-2),
@@ -97,11 +101,25 @@ __device__ void dst_columns(T *G, const T *So, const T *Se, T *E, int nr, int nz
   }
 }
 
+// Optional phase timers (D.phase_clk != nullptr): thread 0 of CTA 0 accumulates clock64 deltas.
+#define PTEFIT_PHASE(k) do { if (D.phase_clk && tid == 0 && blockIdx.x == 0) { const long long t_ = clock64(); D.phase_clk[k] += t_ - t_phase; t_phase = t_; } } while (0)
+
+__device__ __forceinline__ void cp_async4(void *smem, const void *gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
 // grid min(B, resident CTAs), block FUSED_THREADS, dyn smem fused_smem_bytes<T>(nr, nz).
 // cur[B][N] node currents (A), pbd[B][nbnd] boundary flux, psi[B][N] in/out.
 // do_search = 0: Delta* solve only (debug hook); 1: also search + xn (+ dzc when has_delz).
 template <typename T>
-__global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, const T *__restrict__ cur_all,
+__global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int B, const T *__restrict__ cur_all,
                                                                 const T *__restrict__ pbd_all, T *__restrict__ psi_all,
                                                                 T *__restrict__ xn_all, int use_relax, int add_coil,
                                                                 int do_search) {
@@ -112,10 +130,12 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
   T *So = G + ((N + 3) & ~3);
   T *Se = So + n2 * n2;
   T *E = Se + n2 * n2;
+  unsigned *mbits = reinterpret_cast<unsigned *>(E);        // during the search: lim bits, then xpt bits
+  const int nwords = (N + 31) >> 5;
   for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];      // So then Se, contiguous
   // per-column constants (same expressions as the unfused kernels, evaluated once per CTA)
   __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
-  __shared__ T pcoef[2][PTEFIT_MAX_DEG + 1];                 // I'(x) = rdA P(x) + fdA Q(x)
+  __shared__ T pcoef[2 * (PTEFIT_MAX_DEG + 1)];              // I'(x) = rdA P(x) + fdA Q(x)
   __shared__ T c_edge[2];
   for (int i = tid; i < nr; i += nth) {
     const double Rd = D.rmin + i * D.dr;
@@ -129,11 +149,37 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
   const T cz = T(1.0 / (D.dz * D.dz));
   const T scale = T(2.0 / Nz);
   const T om = T(D.relax);
+  const double sg = (double)D.ip_sign;
+  long long t_phase = clock64();
   for (int s = blockIdx.x; s < B; s += gridDim.x) {
     const T *I = cur_all + (size_t)s * N;
     const T *pb = pbd_all + (size_t)s * D.nbnd;           // bottom[nr], top[nr], left[nzi], right[nzi]
     T *psi = psi_all + (size_t)s * N;
+    const T *pc = D.psi_coil + (size_t)s * N;
     __syncthreads();                                       // previous slice done with G; tables loaded
+    // ---- node currents straight into shared memory (asynchronous copies, no register staging)
+    for (int n = tid; n < N; n += nth) {
+      if (sizeof(T) == 4) cp_async4(G + n, I + n); else cp_async8(G + n, I + n);
+    }
+    // inputs of the later phases: pull them into L2 while the solve runs
+    {
+      const int lines = (int)(((size_t)N * sizeof(T) + 127) / 128);
+      for (int l = tid; l < lines; l += nth) {
+        if (add_coil) prefetch_l2(reinterpret_cast<const char *>(pc) + (size_t)l * 128);
+        if (use_relax) prefetch_l2(reinterpret_cast<const char *>(psi) + (size_t)l * 128);
+      }
+    }
+    if (do_search && D.has_delz && tid < 2 * (PTEFIT_MAX_DEG + 1)) {
+      // the P'/FF' sums of I' = J_b(x) X are polynomials in x: collect their coefficients
+      const int kind = tid / (PTEFIT_MAX_DEG + 1), k = tid - kind * (PTEFIT_MAX_DEG + 1);
+      const double *Xp = D.X + (size_t)s * D.nt;
+      double c = 0.0;
+      for (int l = 0; l < D.npoly; ++l)
+        if (D.terms[l].kind == kind) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+      pcoef[tid] = T(c);
+    }
+    cp_async_wait_all();
+    __syncthreads();
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
     {
       int j = tid / nr, i = tid - j * nr;
@@ -144,7 +190,7 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
         else if (i == 0) v = pb[2 * nr + j - 1];
         else if (i == nr - 1) v = pb[2 * nr + nzi + j - 1];
         else {
-          v = c_rhs[i] * I[n];
+          v = c_rhs[i] * G[n];
           if (i == 1) v -= c_edge[0] * pb[2 * nr + j - 1];
           if (i == nri) v -= c_edge[1] * pb[2 * nr + nzi + j - 1];
           if (j == 1) v -= cz * pb[i];
@@ -156,8 +202,11 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
       }
     }
     __syncthreads();
+    PTEFIT_PHASE(0);
     dst_columns<T>(G, So, Se, E, nr, nz);
-    // ---- Thomas sweeps along R in FP64, one thread per mode (precomputed factors)
+    PTEFIT_PHASE(1);
+    // ---- Thomas sweeps along R in FP64, one thread per mode (precomputed factors).
+    // The dependent chain is one DFMA per step.
     if (tid < nzi) {
       const int mm = tid;
       T *row = G + (mm + 1) * nr + 1;
@@ -165,7 +214,7 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
       const double *__restrict__ tw = D.tri_w + mm;
       const double *__restrict__ tb = D.tri_invb + mm;
       const double *__restrict__ tce = D.tri_ce;
-      constexpr int U = 8;                     // factor loads of U steps are issued before the chain
+      constexpr int U = 8;                     // loads of U steps are issued before the dependent chain
       double prev = 0.0;
       for (int i0 = 0; i0 < nri; i0 += U) {
         double w[U];
@@ -174,89 +223,98 @@ __global__ void __launch_bounds__(FUSED_THREADS) k_solve_fused(Dev<T> D, int B, 
 #pragma unroll
         for (int u = 0; u < U; ++u)
           if (i0 + u < nri) {
-            const double v = (double)row[i0 + u] - w[u] * prev;
+            const double v = fma(-w[u], prev, (double)row[i0 + u]);
             y[(size_t)(i0 + u) * nzi] = v;
             prev = v;
           }
       }
       double x = 0.0;
       for (int i0 = nri - 1; i0 >= 0; i0 -= U) {
-        double yy[U], ib[U], ce[U];
+        double a[U], b[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
           const int i = i0 - u;
-          yy[u] = i >= 0 ? y[(size_t)i * nzi] : 0.0;
-          ib[u] = i >= 0 ? __ldg(tb + (size_t)i * nzi) : 0.0;
-          ce[u] = i >= 0 ? __ldg(tce + i) : 0.0;
+          const double ib = i >= 0 ? __ldg(tb + (size_t)i * nzi) : 0.0;
+          a[u] = i >= 0 ? y[(size_t)i * nzi] * ib : 0.0;
+          b[u] = i >= 0 ? __ldg(tce + i) * ib : 0.0;
         }
 #pragma unroll
         for (int u = 0; u < U; ++u)
           if (i0 - u >= 0) {
-            x = (yy[u] - ce[u] * x) * ib[u];
+            x = fma(-b[u], x, a[u]);                       // x_i = (y_i - ce_i x_{i+1}) / piv_i
             row[i0 - u] = T(x);
           }
       }
     }
     __syncthreads();
+    PTEFIT_PHASE(2);
     dst_columns<T>(G, So, Se, E, nr, nz);
-    // ---- total flux + relaxation; psi goes to global memory and stays in G for the search
-    const T *pc = D.psi_coil + (size_t)s * N;
+    PTEFIT_PHASE(3);
+    // ---- bit masks of the search into the (now free) fold buffer
+    if (do_search)
+      for (int w = tid; w < 2 * nwords; w += nth) mbits[w] = (w < nwords) ? D.lim_bits[w] : D.xpt_bits[w - nwords];
+    __syncthreads();
+    // ---- total flux + relaxation; psi goes to global memory and stays in G for the search.
+    // Global loads are issued in batches of EB before use; pass 0 of the search (finiteness and
+    // arg-max over the limiter mask) rides along.
+    SearchOpt<T> so_opt;
+    so_opt.am.v = -INFINITY; so_opt.am.n = 0x7fffffff;
     {
+      constexpr int EB = 8;
       int j = tid / nr, i = tid - j * nr;
-      for (int n = tid; n < N; n += nth) {
-        const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
-        T v = edge ? G[n] : G[n] * scale;
-        if (add_coil) v += pc[n];
-        if (use_relax) { const T old = psi[n]; v = old + om * (v - old); }
-        psi[n] = v;
-        G[n] = v;
-        i += nth;
-        while (i >= nr) { i -= nr; ++j; }
+      for (int n0 = tid; n0 < N; n0 += EB * nth) {
+        T cv[EB], ov[EB];
+#pragma unroll
+        for (int u = 0; u < EB; ++u) {
+          const int n = n0 + u * nth;
+          cv[u] = (add_coil && n < N) ? pc[n] : T(0);
+          ov[u] = (use_relax && n < N) ? psi[n] : T(0);
+        }
+#pragma unroll
+        for (int u = 0; u < EB; ++u) {
+          const int n = n0 + u * nth;
+          if (n < N) {
+            const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
+            T v = edge ? G[n] : G[n] * scale;
+            v += cv[u];
+            if (use_relax) v = ov[u] + om * (v - ov[u]);
+            psi[n] = v;
+            G[n] = v;
+            if (do_search) {
+              const double dv = (double)v;
+              so_opt.bad |= !isfinite(dv);
+              if ((mbits[n >> 5] >> (n & 31)) & 1u) { ArgMax c; c.v = sg * dv; c.n = n; so_opt.am = better(so_opt.am, c); }
+            }
+            i += nth;
+            while (i >= nr) { i -= nr; ++j; }
+          }
+        }
       }
     }
     __syncthreads();
+    PTEFIT_PHASE(4);
     if (do_search) {
       T *xn = xn_all + (size_t)s * N;
-      search_body<T>(D, s, G, xn, G);                      // G now holds xn
+      so_opt.lbits = mbits; so_opt.xbits = mbits + nwords; so_opt.have_am = true;
+      so_opt.local = G;
+      if (D.has_delz) { so_opt.pc = pcoef; so_opt.rdA = c_rdA; so_opt.fdA = c_fdA; }
+      search_body<T>(D, s, G, xn, so_opt);                 // G now holds I'(xn) (delz) or xn
+      PTEFIT_PHASE(5);
       if (D.has_delz) {
-        // -dI'/dZ column for the NEXT fit: I' = J_b(xn) X with the coefficients of this fit.
-        // The P'/FF' sums are polynomials in x: collect their coefficients once per slice,
-        // evaluate I' per node by Horner in place of xn, then difference along Z.
-        if (tid < 2 * (PTEFIT_MAX_DEG + 1)) {
-          const int kind = tid / (PTEFIT_MAX_DEG + 1), k = tid - kind * (PTEFIT_MAX_DEG + 1);
-          const double *Xp = D.X + (size_t)s * D.nt;
-          double c = 0.0;
-          for (int l = 0; l < D.npoly; ++l)
-            if (D.terms[l].kind == kind) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
-          pcoef[kind][k] = T(c);
-        }
-        __syncthreads();
-        {
-          int j = tid / nr, i = tid - j * nr;
-          for (int n = tid; n < N; n += nth) {
-            const T x = G[n];
-            T hp = pcoef[0][PTEFIT_MAX_DEG], hq = pcoef[1][PTEFIT_MAX_DEG];
-#pragma unroll
-            for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fma(hp, x, pcoef[0][k]); hq = fma(hq, x, pcoef[1][k]); }
-            G[n] = (x < T(0)) ? T(0) : fma(c_rdA[i], hp, c_fdA[i] * hq);
-            i += nth;
-            while (i >= nr) { i -= nr; ++j; }
-          }
-        }
+        // -dI'/dZ column for the NEXT fit (I' = J_b(xn) X with the coefficients of this fit)
         __syncthreads();
         T *dzc = D.dzc + (size_t)s * N;
         const T hz = T(0.5 / D.dz);
-        {
-          int j = tid / nr, i = tid - j * nr;
-          for (int n = tid; n < N; n += nth) {
-            T out = T(0);
-            if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) out = -(G[n + nr] - G[n - nr]) * hz;
-            dzc[n] = out;
-            i += nth;
-            while (i >= nr) { i -= nr; ++j; }
-          }
+        int j = tid / nr, i = tid - j * nr;
+        for (int n = tid; n < N; n += nth) {
+          T out = T(0);
+          if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) out = -(G[n + nr] - G[n - nr]) * hz;
+          dzc[n] = out;
+          i += nth;
+          while (i >= nr) { i -= nr; ++j; }
         }
       }
+      PTEFIT_PHASE(6);
     }
   }
 }

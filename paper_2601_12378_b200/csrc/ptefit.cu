@@ -28,6 +28,7 @@ struct ptefit_handle {
   std::vector<void *> allocs;
   std::string error;
   int launches = 0;
+  long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
   int fused_grid = 0;                   // resident CTAs of k_solve_fused
   size_t fused_smem = 0;
@@ -97,7 +98,7 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   D.dr = (g->rmax - g->rmin) / (g->nr - 1); D.dz = (g->zmax - g->zmin) / (g->nz - 1);
   D.dA = D.dr * D.dz; D.lambda_reg = ba->lambda_reg; D.relax = ba->relax;
   D.cold_rc = ge->cold_rc; D.cold_zc = ge->cold_zc; D.cold_a = ge->cold_a; D.cold_b = ge->cold_b;
-  D.npoly = 0; D.has_delz = 0;
+  D.npoly = 0; D.has_delz = 0; D.phase_clk = nullptr;
   for (int l = 0; l < ba->n_terms; ++l) {
     D.terms[l].kind = ba->terms[l].kind; D.terms[l].i = ba->terms[l].i; D.terms[l].N = ba->terms[l].N;
     if (ba->terms[l].kind == 2) D.has_delz = 1; else D.npoly++;
@@ -125,6 +126,16 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   }
   TRY(upload(h, &D.lim_mask, ge->lim_mask, N));
   TRY(upload(h, &D.xpt_mask, ge->xpt_mask ? ge->xpt_mask : ge->lim_mask, N));
+  {
+    const unsigned char *xm = ge->xpt_mask ? ge->xpt_mask : ge->lim_mask;
+    std::vector<unsigned> lb((N + 31) / 32, 0u), xb((N + 31) / 32, 0u);
+    for (size_t n = 0; n < N; ++n) {
+      if (ge->lim_mask[n]) lb[n >> 5] |= 1u << (n & 31);
+      if (xm[n]) xb[n >> 5] |= 1u << (n & 31);
+    }
+    TRY(upload(h, &D.lim_bits, lb.data(), lb.size()));
+    TRY(upload(h, &D.xpt_bits, xb.data(), xb.size()));
+  }
   TRY(upload(h, &D.lim_r, ge->lim_r, (size_t)D.nlim));
   TRY(upload(h, &D.lim_z, ge->lim_z, (size_t)D.nlim));
   // Delta* factors ("the coefficient matrices can be pre-computed"): for each DST
@@ -250,6 +261,7 @@ extern "C" void ptefit_destroy(ptefit_handle *h) {
   for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   void *hp[] = {h->hb, h->hic, h->hpsi, h->hco, h->hax, h->hxp, h->hpb, h->hchi, h->haxij, h->hxpij, h->hlim, h->hst};
   for (void *p : hp) if (p) cudaFree(p);
+  if (h->phase_clk) cudaFree(h->phase_clk);
   if (h->hstream) cudaStreamDestroy(h->hstream);
   delete h;
 }

@@ -64,14 +64,27 @@ __device__ __forceinline__ ArgMax block_argmax(ArgMax a, ArgMax *sh) {
   return r;
 }
 
+// Optional shared-memory helpers of search_body (all nullptr / default = plain global-memory path).
+template <typename T>
+struct SearchOpt {
+  const unsigned *lbits = nullptr;   // bit-packed lim_mask in shared memory (bit n&31 of word n>>5)
+  const unsigned *xbits = nullptr;   // bit-packed xpt_mask
+  bool have_am = false;              // pass 0 done by the caller: this thread's partial arg-max + finiteness
+  ArgMax am;
+  bool bad = false;
+  T *local = nullptr;                // per-node output in shared memory (may alias psi)
+  const T *pc = nullptr;             // if set: local gets I'(xn) = rdA P(xn) + fdA Q(xn) instead of xn
+  const T *rdA = nullptr, *fdA = nullptr;
+};
+
 // Search of one slice by one CTA (any block size that is a multiple of 32, <= 1024).  Reads
 // psi[nz][nr] (global or shared memory), writes xn (normalised flux in the mask, -1 outside) to
-// global memory and, if xn_local != nullptr, also to xn_local (may alias psi: every thread
-// overwrites only nodes it alone reads after the last barrier).  Updates D.so[s], D.status[s]
-// (sticky).  All threads of the CTA must call it.
+// global memory and, if o.local != nullptr, a per-node value to o.local (may alias psi: every
+// thread overwrites only nodes it alone reads after the last barrier).  Updates D.so[s],
+// D.status[s] (sticky).  All threads of the CTA must call it.
 template <typename T>
-__device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, T *xn_local) {
-  const int nth = blockDim.x;
+__device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, const SearchOpt<T> &o) {
+  const int nth = blockDim.x, tid = threadIdx.x;
   const int nr = D.nr, N = D.N;
   const double sg = (double)D.ip_sign;
   __shared__ ArgMax sh_am[32];
@@ -79,16 +92,19 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   __shared__ double cR[PTEFIT_MAX_CAND], cZ[PTEFIT_MAX_CAND], cP[PTEFIT_MAX_CAND];
   __shared__ int cN[PTEFIT_MAX_CAND];
   __shared__ SearchOut so;
-  __shared__ int sh_status;
-  if (threadIdx.x == 0) { sh_flag = 0; sh_ncand = 0; sh_count = 0; sh_status = 0; }
+  if (tid == 0) { sh_flag = 0; sh_ncand = 0; sh_count = 0; }
   __syncthreads();
   // 0. finiteness + 1. axis node: arg-max of s*psi over lim_mask, tie -> smallest n
   ArgMax am; am.v = -INFINITY; am.n = 0x7fffffff;
   bool bad = false;
-  for (int n = threadIdx.x; n < N; n += nth) {
-    const double v = (double)psi[n];
-    bad |= !isfinite(v);
-    if (D.lim_mask[n]) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
+  if (o.have_am) { am = o.am; bad = o.bad; }
+  else {
+    for (int n = tid; n < N; n += nth) {
+      const double v = (double)psi[n];
+      bad |= !isfinite(v);
+      const bool lm = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
+      if (lm) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
+    }
   }
   if (bad) atomicOr(&sh_flag, 1);
   am = block_argmax(am, sh_am);
@@ -104,10 +120,14 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   }
   // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
   if (status == 0) {
-    for (int n = threadIdx.x; n < N; n += nth) {
-      if (!D.xpt_mask[n]) continue;
+    for (int n = tid; n < N; n += nth) {
+      const bool xm = o.xbits ? ((o.xbits[n >> 5] >> (n & 31)) & 1u) : D.xpt_mask[n];
+      if (!xm) continue;
       const Quad qc = quad_coef(psi + n, nr);
-      if (!(qc.det < 0.0)) continue;                  // the divisions only for saddle-like nodes
+      if (!(qc.det < 0.0)) continue;
+      // division-free pre-test with a margin; the decision itself is taken below on x*, y*
+      const double lim = 0.5000001 * fabs(qc.det);
+      if (fabs(2.0 * qc.cyy * qc.cx - qc.cxy * qc.cy) > lim || fabs(2.0 * qc.cxx * qc.cy - qc.cxy * qc.cx) > lim) continue;
       const Fit f = quad_finish(qc);
       if (f.det < 0.0 && fabs(f.xs) <= 0.5 && fabs(f.ys) <= 0.5 && sg * f.ps < sg * Pa) {
         const int q = atomicAdd(&sh_ncand, 1);
@@ -124,7 +144,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   // 3. limiter vertices: bilinear flux, valid iff not behind any candidate as seen from the axis
   ArgMax lm; lm.v = -INFINITY; lm.n = 0x7fffffff;
   if (status == 0) {
-    for (int v = threadIdx.x; v < D.nlim; v += nth) {
+    for (int v = tid; v < D.nlim; v += nth) {
       const double lr = D.lim_r[v], lz = D.lim_z[v];
       const double fi = (lr - D.rmin) / D.dr, fj = (lz - D.zmin) / D.dz;
       int i0 = (int)floor(fi), j0 = (int)floor(fj);
@@ -153,7 +173,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     const double spb = xwins ? bx.v : lm.v;
     if (!isfinite(spb)) status = 1;
     Pb = sg * spb;
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
       so.axis_i = ia; so.axis_j = ja; so.axis_r = Ra; so.axis_z = Za; so.axis_psi = Pa;
       so.n_cand = ncand; so.limited = xwins ? 0 : 1; so.psi_b = Pb;
       if (qbest >= 0) {
@@ -169,29 +189,49 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   int cnt = 0;
   if (status == 0) {
     const double inv = 1.0 / (Pb - Pa);
-    for (int n = threadIdx.x; n < N; n += nth) {
+    int j = tid / nr, i = tid - j * nr;
+    for (int n = tid; n < N; n += nth) {
       T out = T(-1);
-      if (D.lim_mask[n]) {
+      const bool lmk = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
+      if (lmk) {
         const double v = (double)psi[n];
         if (sg * (v - Pb) > 0.0) {
-          const int j = n / nr, i = n - j * nr;
-          const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
           bool in = true;
-          for (int c = 0; c < ncand; ++c)
-            in &= ((R - cR[c]) * (Ra - cR[c]) + (Z - cZ[c]) * (Za - cZ[c])) > 0.0;
+          if (ncand) {
+            const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
+            for (int c = 0; c < ncand; ++c)
+              in &= ((R - cR[c]) * (Ra - cR[c]) + (Z - cZ[c]) * (Za - cZ[c])) > 0.0;
+          }
           if (in) { out = T(fmin(fmax((v - Pa) * inv, 0.0), 1.0)); ++cnt; }
         }
       }
       xn[n] = out;
-      if (xn_local) xn_local[n] = out;
+      if (o.local) {
+        T lv = out;
+        if (o.pc) {                                   // I'(x) by Horner (fused_solve.cuh, delz column)
+          T hp = o.pc[PTEFIT_MAX_DEG], hq = o.pc[2 * PTEFIT_MAX_DEG + 1];
+#pragma unroll
+          for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) {
+            hp = fma(hp, out, o.pc[k]);
+            hq = fma(hq, out, o.pc[PTEFIT_MAX_DEG + 1 + k]);
+          }
+          lv = (out < T(0)) ? T(0) : fma(o.rdA[i], hp, o.fdA[i] * hq);
+        }
+        o.local[n] = lv;
+      }
+      i += nth;
+      while (i >= nr) { i -= nr; ++j; }
     }
-  } else if (xn_local) {
-    for (int n = threadIdx.x; n < N; n += nth) xn_local[n] = T(-1);
+  } else {
+    for (int n = tid; n < N; n += nth) {
+      xn[n] = T(-1);
+      if (o.local) o.local[n] = o.pc ? T(0) : T(-1);
+    }
   }
   if (cnt) atomicAdd(&sh_count, cnt);
   __syncthreads();
   if (status == 0 && sh_count == 0) status = 1;
-  if (threadIdx.x == 0) {
+  if (tid == 0) {
     if (D.status[s] == 0) {
       if (status == 0 || status == 4) D.so[s] = so;
       if (status == 1 || status == 2) { SearchOut z = {}; z.axis_i = ia; z.axis_j = ja; z.xpt_i = z.xpt_j = -1; D.so[s] = z; }
@@ -205,7 +245,8 @@ template <typename T>
 __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__restrict__ psi_all,
                                                             T *__restrict__ xn_all) {
   const int s = blockIdx.x;
-  search_body<T>(D, s, psi_all + (size_t)s * D.N, xn_all + (size_t)s * D.N, nullptr);
+  SearchOpt<T> o;
+  search_body<T>(D, s, psi_all + (size_t)s * D.N, xn_all + (size_t)s * D.N, o);
 }
 
 // Copy the per-slice search results and fit outputs to the caller's arrays.  grid ceil(B/128).
