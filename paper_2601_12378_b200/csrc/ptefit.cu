@@ -5,8 +5,10 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "common.cuh"
@@ -14,6 +16,8 @@
 #include "search_kernels.cuh"
 #include "solve_kernels.cuh"
 #include "fused_solve.cuh"
+#include "tc_gemm.cuh"
+#include "tc_kernels.cuh"
 
 using namespace ptefit;
 
@@ -28,6 +32,11 @@ struct ptefit_handle {
   std::vector<void *> allocs;
   std::string error;
   int launches = 0;
+  bool tc = false;                      // tensor-core contractions usable (FP32, 3xTF32 mode)
+  TcDev Tc{};
+  const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;
+  int pbd_ntiles = 0;
+  CUtensorMap mapJbHi, mapJbLo, mapGpHi, mapGpLo, mapCurHi, mapCurLo, mapGbHi, mapGbLo;
   long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
   int fused_grid = 0;                   // resident CTAs of k_solve_fused
@@ -200,6 +209,8 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   return PTEFIT_OK;
 }
 
+#include "tc_host.inc"
+
 extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geometry *ge,
                                        const ptefit_tables *tb, const ptefit_basis *ba,
                                        const ptefit_options *op, ptefit_handle **out) {
@@ -250,6 +261,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   h->prec = op->precision; h->gemm = op->gemm; h->max_batch = op->max_batch;
   ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
                                               : build(h, h->d64, g, ge, tb, ba, op->max_batch);
+  if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) st = build_tc(h, h->d32, ge, tb, op->max_batch);
   if (st != PTEFIT_OK) { std::string e = h->error; ptefit_destroy(h); g_error = e; return st; }
   *out = h;
   return PTEFIT_OK;

@@ -1,0 +1,251 @@
+// tc_gemm.cuh -- the two dense contractions of the Picard iteration on the 5th-generation tensor
+// cores (tcgen05.mma kind::tf32, accumulators in TMEM, operands staged by TMA):
+//   response  R = G_P J_b            (Eq. 6)   rows = (slice, term), cols = channels
+//   boundary  psi_bdry = G_B I       (Dirichlet data)   rows = slices, cols = edge nodes
+// Both are D[M][N] = A[M][K] B[N][K]^T with K = the compacted list of nodes that may carry current
+// (lim_mask = 1), A = per-slice data, B = a Green's table.  FP32 accuracy comes from the 3xTF32
+// split a = a_hi + a_lo (a_hi = a rounded to TF32):  D += A_hi B_hi + A_hi B_lo + A_lo B_hi.
+// K is split over blockIdx.z; each split writes its own partial (summed in a fixed order by the
+// consumer, so results are bit-reproducible).  DESIGN.md "k_gemm_3xtf32".
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ptefit {
+namespace tc {
+
+constexpr int BM = 128;          // rows of A per CTA (TMEM lanes)
+constexpr int BK = 32;           // K per stage: 32 floats = one 128-byte swizzle row
+constexpr int UMMA_K = 8;        // K of one tcgen05.mma kind::tf32
+constexpr int GEMM_THREADS = 320;  // warp 0: TMA, warp 1: MMA, warps 2-9: accumulate + epilogue
+constexpr int DRAIN = 4;         // K blocks accumulated in TMEM before promotion to FP32 registers
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
+// 2-D TMA tile load: coordinates (c0 = innermost = k, c1 = row), completion on an mbarrier.
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n" ::"r"(smem_u32(dst)),
+      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap *map) {
+  asm volatile("prefetch.tensormap [%0];\n" ::"l"(map) : "memory");
+}
+
+// TMEM allocation (one warp), columns = power of two >= 32.
+template <int COLS>
+__device__ __forceinline__ void tmem_alloc(uint32_t *slot) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(slot)), "n"(COLS));
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n");
+}
+template <int COLS>
+__device__ __forceinline__ void tmem_dealloc(uint32_t addr) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(addr), "n"(COLS));
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// Shared-memory matrix descriptor, K-major operand, 128-byte swizzle: rows are 128 bytes, groups of
+// 8 rows (1024 bytes) follow each other (stride byte offset 1024); sm_100 descriptor version 1.
+__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);            // start address, bits [0,14)
+  d |= (uint64_t)1 << 16;                              // leading byte offset (unused with swizzle)
+  d |= (uint64_t)(1024 >> 4) << 32;                    // stride byte offset, bits [32,46)
+  d |= (uint64_t)1 << 46;                              // version = 1 (Blackwell)
+  d |= (uint64_t)2 << 61;                              // layout: SWIZZLE_128B
+  return d;
+}
+// Instruction descriptor: D = F32, A = B = TF32, both K-major, shape M x N.
+__host__ __device__ constexpr uint32_t idesc_tf32(int M, int N) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// TMEM -> registers: this warp's 32 lanes x 16 consecutive 32-bit columns.
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float *v) {
+  uint32_t r[16];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+  for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
+}
+
+
+template <int BN, int STAGES>
+struct GemmSmem {
+  static constexpr int A_BYTES = BM * BK * 4;            // 16 KB per hi / lo tile
+  static constexpr int B_BYTES = BN * BK * 4;
+  static constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;
+  static constexpr int BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+};
+
+// D partial[z][m][n] = sum over the K blocks of split z of A[m][k] B[n][k]  (3xTF32).
+// The tensor core adds into its TMEM accumulator with truncation, so long accumulation chains drift
+// (measured: 1e-5 relative after ~700 MMAs).  The chain is therefore cut every DRAIN K blocks: the
+// MMA warp alternates between two TMEM accumulators, and the eight accumulate warps add each
+// finished chunk into FP32 registers (round-to-nearest) while the next chunk is being multiplied.
+// grid (M tiles, N tiles, splits), block GEMM_THREADS, dyn smem GemmSmem<BN,STAGES>::BYTES.
+// out: [splits][m_rows][ldo] floats, m_rows = gridDim.x * BM, ldo >= gridDim.y * BN.
+template <int BN, int STAGES>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant__ CUtensorMap mapAlo,
+              const __grid_constant__ CUtensorMap mapBhi, const __grid_constant__ CUtensorMap mapBlo,
+              float *__restrict__ out, int ldo, int kblocks) {
+  using L = GemmSmem<BN, STAGES>;
+  static_assert(BN % 16 == 0 && BN <= 256, "N tile");
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char *base = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint64_t *full = reinterpret_cast<uint64_t *>(base + STAGES * L::STAGE_BYTES);
+  uint64_t *empty = full + STAGES;
+  uint64_t *tfull = empty + STAGES;                    // [2] accumulator chunk ready
+  uint64_t *tempty = tfull + 2;                        // [2] accumulator drained
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  const int nsplit = gridDim.z, z = blockIdx.z;
+  const int kb0 = (int)(((long long)kblocks * z) / nsplit), kb1 = (int)(((long long)kblocks * (z + 1)) / nsplit);
+  const int nchunks = (kb1 - kb0 + DRAIN - 1) / DRAIN;
+  constexpr int ACC_COLS = BN <= 64 ? 64 : BN <= 128 ? 128 : 256;      // column stride between the two accumulators
+  constexpr int TMEM_COLS = 2 * ACC_COLS;
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&mapAhi); tma_prefetch_desc(&mapAlo); tma_prefetch_desc(&mapBhi); tma_prefetch_desc(&mapBlo);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 8); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<TMEM_COLS>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {                                   // ---- TMA producer
+      for (int kb = kb0, it = 0; kb < kb1; ++kb, ++it) {
+        const int s = it % STAGES;
+        const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
+        mbar_wait(empty + s, ph ^ 1u);
+        unsigned char *st = base + s * L::STAGE_BYTES;
+        mbar_expect_tx(full + s, (uint32_t)L::STAGE_BYTES);
+        tma_load_2d(st, &mapAhi, full + s, kb * BK, m0);
+        tma_load_2d(st + L::A_BYTES, &mapAlo, full + s, kb * BK, m0);
+        tma_load_2d(st + 2 * L::A_BYTES, &mapBhi, full + s, kb * BK, n0);
+        tma_load_2d(st + 2 * L::A_BYTES + L::B_BYTES, &mapBlo, full + s, kb * BK, n0);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {                                   // ---- MMA issuer
+      constexpr uint32_t idesc = idesc_tf32(BM, BN);
+      int it = 0;
+      for (int c = 0; c < nchunks; ++c) {
+        const int buf = c & 1;
+        mbar_wait(tempty + buf, ((uint32_t)(c >> 1) & 1u) ^ 1u);       // accumulator drained by the register adders
+        tc_fence_after();
+        const uint32_t tacc = tmem_base + (uint32_t)(buf * ACC_COLS);
+        const int kend = min(kb0 + (c + 1) * DRAIN, kb1);
+        for (int kb = kb0 + c * DRAIN; kb < kend; ++kb, ++it) {
+          const int s = it % STAGES;
+          const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
+          mbar_wait(full + s, ph);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(base + s * L::STAGE_BYTES);
+          const uint64_t dAhi = smem_desc_sw128(sa), dAlo = smem_desc_sw128(sa + L::A_BYTES);
+          const uint64_t dBhi = smem_desc_sw128(sa + 2 * L::A_BYTES), dBlo = smem_desc_sw128(sa + 2 * L::A_BYTES + L::B_BYTES);
+#pragma unroll
+          for (int k = 0; k < BK / UMMA_K; ++k) {
+            const uint64_t adv = (uint64_t)((k * UMMA_K * 4) >> 4);    // +32 bytes per K step inside the swizzle row
+            // small terms first, so that they are not absorbed by the large one
+            mma_tf32(tacc, dAlo + adv, dBhi + adv, idesc, (kb > kb0 + c * DRAIN || k > 0) ? 1u : 0u);
+            mma_tf32(tacc, dAhi + adv, dBlo + adv, idesc, 1u);
+            mma_tf32(tacc, dAhi + adv, dBhi + adv, idesc, 1u);
+          }
+          tc_commit(empty + s);                        // frees the stage once these MMAs have read it
+        }
+        tc_commit(tfull + buf);                        // chunk complete
+      }
+    }
+  } else {                                             // ---- promotion to registers + epilogue
+    const int q = warp & 3;                            // TMEM lane quarter this warp may access
+    const int half = (warp - 2) >> 2;                  // which half of the columns
+    constexpr int C0 = ((BN / 16 + 1) / 2) * 16;       // columns of half 0 (multiple of 16)
+    constexpr int NCH = C0 / 16;                       // 16-column groups per thread (half 1 may use fewer)
+    const int col0 = half ? C0 : 0, ncols = half ? BN - C0 : C0;
+    float acc[NCH][16];
+#pragma unroll
+    for (int g = 0; g < NCH; ++g)
+#pragma unroll
+      for (int k = 0; k < 16; ++k) acc[g][k] = 0.f;
+    for (int c = 0; c < nchunks; ++c) {
+      const int buf = c & 1;
+      mbar_wait(tfull + buf, (uint32_t)(c >> 1) & 1u);
+      tc_fence_after();
+      const uint32_t tacc = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * ACC_COLS + col0);
+#pragma unroll
+      for (int g = 0; g < NCH; ++g) {
+        if (g * 16 < ncols) {
+          float v[16];
+          tmem_ld16(tacc + (uint32_t)(g * 16), v);
+#pragma unroll
+          for (int k = 0; k < 16; ++k) acc[g][k] += v[k];
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty + buf);
+    }
+    const int row = q * 32 + lane;
+    float *o = out + ((size_t)z * gridDim.x * BM + m0 + row) * ldo + n0 + col0;
+#pragma unroll
+    for (int g = 0; g < NCH; ++g) {
+      if (g * 16 < ncols) {
+#pragma unroll
+        for (int k = 0; k < 16; k += 4)
+          *reinterpret_cast<float4 *>(o + g * 16 + k) = make_float4(acc[g][k], acc[g][k + 1], acc[g][k + 2], acc[g][k + 3]);
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc<TMEM_COLS>(tmem_base);
+}
+
+}  // namespace tc
+}  // namespace ptefit
