@@ -165,11 +165,11 @@ def stage_roofline(stage, ms_per_launch, dims, peaks, gemm_mode):
     tf32 = 0.5 * peaks["bf16_sustained"]           # guide: nominal TF32 dense = 1/2 of bf16 dense
     if stage == "response":
         flops = 2.0 * M * Nint * nt * B
-        return dict(kernel="k_response", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
+        return dict(kernel="k_basis_split+k_gemm_3xtf32<144,3>+k_resp_reduce", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
                     unit="TFLOP/s", peak_note=f"0.5 x measured sustained bf16 ({peaks['source']}); gemm mode {gemm_mode}")
     if stage == "boundary":
         flops = 2.0 * Nb * Nint * B
-        return dict(kernel="k_boundary", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
+        return dict(kernel="k_cur_split+k_gemm_3xtf32<256,2>+k_pbd_reduce", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
                     unit="TFLOP/s", peak_note=f"0.5 x measured sustained bf16 ({peaks['source']}); gemm mode {gemm_mode}")
     if stage == "solve" and dims.get("fused"):
         # k_solve_fused: read I, psi_coil, old psi; write psi, normalised flux, delz column (+ boundary flux)
@@ -362,7 +362,7 @@ def main():
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--batch", type=int, default=0, help="override the config's batch")
     ap.add_argument("--unique", type=int, default=128, help="distinct seeded slices per rank (tiled to the batch)")
-    ap.add_argument("--gemm", default="ffma", help="contraction arithmetic label recorded in config")
+    ap.add_argument("--gemm", default="3xtf32", help="contraction arithmetic label recorded in config")
     ap.add_argument("--cpu-sample", type=int, default=24, help="slices the cpu_baseline leg times")
     ap.add_argument("--skip-extras", action="store_true", help="timed region + stage breakdown only (for ncu runs)")
     ap.add_argument("--ref-sample", type=int, default=4, help="--impl reference: slices per step")

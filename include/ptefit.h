@@ -142,9 +142,10 @@ ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
 
 /* In-kernel phase timers of k_solve_fused (tuning aid): on = 1 enables them (one CTA's thread 0
  * accumulates SM-clock cycles per phase: 0 rhs, 1 DST, 2 Thomas, 3 DST, 4 total flux, 5 search,
- * 6 delz column); with out != NULL the accumulated cycles are copied to out[8] (HOST) and
- * reset.  Synchronises the device. */
-ptefit_status ptefit_debug_phase_clocks(ptefit_handle *h, int on, long long out[8]);
+ * 6 delz column; 8..13 sub-phases of the search: arg-max reduce, axis fit, candidates, limiter,
+ * boundary flux, mask + normalisation); with out != NULL the accumulated cycles are copied to
+ * out[16] (HOST) and reset.  Synchronises the device. */
+ptefit_status ptefit_debug_phase_clocks(ptefit_handle *h, int on, long long out[16]);
 
 void ptefit_destroy(ptefit_handle *h);
 const char *ptefit_last_error(const ptefit_handle *h);

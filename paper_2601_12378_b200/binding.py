@@ -246,7 +246,7 @@ class Reconstructor:
         return dict(zip(("setup", "response", "lsq", "boundary", "solve", "search"), list(out)))
 
     def phase_clocks(self, on=True, read=False):
-        out = (C.c_longlong * 8)() if read else None
+        out = (C.c_longlong * 16)() if read else None
         self._call(self.lib.ptefit_debug_phase_clocks, int(on), out)
         return list(out) if read else None
 

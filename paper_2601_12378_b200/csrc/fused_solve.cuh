@@ -44,6 +44,8 @@ __host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
   size_t e = 2 * (size_t)n2 * FUSED_CW * sizeof(T);               // fold buffer, reused for the bit masks
   const size_t mb = 2 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);
   if (mb > e) e = mb;
+  const size_t pbb = (size_t)(2 * (nr + nz) - 4) * sizeof(T);   // ... and for the boundary flux
+  if (pbb > e) e = pbb;
   e = (e + 15) & ~(size_t)15;
   return (g + 2 * (size_t)n2 * n2) * sizeof(T) + e;
 }
@@ -153,11 +155,13 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
   long long t_phase = clock64();
   for (int s = blockIdx.x; s < B; s += gridDim.x) {
     const T *I = cur_all + (size_t)s * N;
-    const T *pb = pbd_all + (size_t)s * D.nbnd;           // bottom[nr], top[nr], left[nzi], right[nzi]
+    const T *pbg = pbd_all + (size_t)s * D.nbnd;          // bottom[nr], top[nr], left[nzi], right[nzi]
+    const T *pb = E;                                       // staged in the fold buffer (free until the DST)
     T *psi = psi_all + (size_t)s * N;
     const T *pc = D.psi_coil + (size_t)s * N;
     __syncthreads();                                       // previous slice done with G; tables loaded
     // ---- node currents straight into shared memory (asynchronous copies, no register staging)
+    for (int k = tid; k < D.nbnd; k += nth) E[k] = pbg[k];
     for (int n = tid; n < N; n += nth) {
       if (sizeof(T) == 4) cp_async4(G + n, I + n); else cp_async8(G + n, I + n);
     }
@@ -178,8 +182,10 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
         if (D.terms[l].kind == kind) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
       pcoef[tid] = T(c);
     }
+    PTEFIT_PHASE(14);
     cp_async_wait_all();
     __syncthreads();
+    PTEFIT_PHASE(15);
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
     {
       int j = tid / nr, i = tid - j * nr;
@@ -262,13 +268,22 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     {
       constexpr int EB = 8;
       int j = tid / nr, i = tid - j * nr;
+      T cn[EB], on[EB];                                    // next batch, in flight while this one is used
+#pragma unroll
+      for (int u = 0; u < EB; ++u) {
+        const int n = tid + u * nth;
+        cn[u] = (add_coil && n < N) ? pc[n] : T(0);
+        on[u] = (use_relax && n < N) ? psi[n] : T(0);
+      }
       for (int n0 = tid; n0 < N; n0 += EB * nth) {
         T cv[EB], ov[EB];
 #pragma unroll
+        for (int u = 0; u < EB; ++u) { cv[u] = cn[u]; ov[u] = on[u]; }
+#pragma unroll
         for (int u = 0; u < EB; ++u) {
-          const int n = n0 + u * nth;
-          cv[u] = (add_coil && n < N) ? pc[n] : T(0);
-          ov[u] = (use_relax && n < N) ? psi[n] : T(0);
+          const int n = n0 + (EB + u) * nth;
+          cn[u] = (add_coil && n < N) ? pc[n] : T(0);
+          on[u] = (use_relax && n < N) ? psi[n] : T(0);
         }
 #pragma unroll
         for (int u = 0; u < EB; ++u) {

@@ -82,6 +82,8 @@ struct SearchOpt {
 // global memory and, if o.local != nullptr, a per-node value to o.local (may alias psi: every
 // thread overwrites only nodes it alone reads after the last barrier).  Updates D.so[s],
 // D.status[s] (sticky).  All threads of the CTA must call it.
+#define PTEFIT_SP(k) do { if (D.phase_clk && threadIdx.x == 0 && blockIdx.x == 0) { const long long t_ = clock64(); D.phase_clk[k] += t_ - t_sp; t_sp = t_; } } while (0)
+
 template <typename T>
 __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, const SearchOpt<T> &o) {
   const int nth = blockDim.x, tid = threadIdx.x;
@@ -92,6 +94,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   __shared__ double cR[PTEFIT_MAX_CAND], cZ[PTEFIT_MAX_CAND], cP[PTEFIT_MAX_CAND];
   __shared__ int cN[PTEFIT_MAX_CAND];
   __shared__ SearchOut so;
+  long long t_sp = clock64();
   if (tid == 0) { sh_flag = 0; sh_ncand = 0; sh_count = 0; }
   __syncthreads();
   // 0. finiteness + 1. axis node: arg-max of s*psi over lim_mask, tie -> smallest n
@@ -108,6 +111,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   }
   if (bad) atomicOr(&sh_flag, 1);
   am = block_argmax(am, sh_am);
+  PTEFIT_SP(8);
   int status = 0;
   if (sh_flag) status = 2;
   double Ra = 0, Za = 0, Pa = 0;
@@ -118,11 +122,31 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     if (!(f.det > 0.0) || fmax(fabs(f.xs), fabs(f.ys)) > 1.0) status = 1;
     Ra = D.rmin + (ia + f.xs) * D.dr; Za = D.zmin + (ja + f.ys) * D.dz; Pa = f.ps;
   }
+  PTEFIT_SP(9);
   // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
   if (status == 0) {
     for (int n = tid; n < N; n += nth) {
       const bool xm = o.xbits ? ((o.xbits[n >> 5] >> (n & 31)) & 1u) : D.xpt_mask[n];
       if (!xm) continue;
+      if (sizeof(T) == 4) {
+        // FP32 pre-filter with wide margins (the coefficients carry ~1e-4 relative error in FP32):
+        // skip nodes whose Hessian determinant is certainly positive or whose stationary point is
+        // certainly outside the half cell; everything else is decided below in FP64.
+        const T *p = psi + n;
+        const float a = p[-nr - 1], b = p[-nr], c = p[-nr + 1], d = p[-1], e = p[0], f = p[1], g = p[nr - 1], hh = p[nr], k = p[nr + 1];
+        const float l3 = a + d + g, r3 = c + f + k, m3 = b + e + hh, t3 = a + b + c, u3 = g + hh + k, w3 = d + e + f;
+        const float fcx = (r3 - l3) * (1.f / 6.f), fcy = (u3 - t3) * (1.f / 6.f);
+        const float fcxx = (l3 - 2.f * m3 + r3) * (1.f / 6.f), fcyy = (t3 - 2.f * w3 + u3) * (1.f / 6.f);
+        const float fcxy = (k + a - g - c) * 0.25f;
+        const float p1 = 4.f * fcxx * fcyy, p2 = fcxy * fcxy, fdet = p1 - p2, mag = fabsf(p1) + p2;
+        if (fdet > 0.02f * mag) continue;
+        if (fdet < -0.02f * mag) {
+          const float lim = 0.6f * fabsf(fdet);
+          const float sx = fabsf(fcyy * fcx) + fabsf(fcxy * fcy), sy = fabsf(fcxx * fcy) + fabsf(fcxy * fcx);
+          const float nx = fabsf(2.f * fcyy * fcx - fcxy * fcy), ny = fabsf(2.f * fcxx * fcy - fcxy * fcx);
+          if (nx > lim + 0.02f * sx || ny > lim + 0.02f * sy) continue;
+        }
+      }
       const Quad qc = quad_coef(psi + n, nr);
       if (!(qc.det < 0.0)) continue;
       // division-free pre-test with a margin; the decision itself is taken below on x*, y*
@@ -139,6 +163,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
   }
   __syncthreads();
+  PTEFIT_SP(10);
   const int ncand = sh_ncand;
   if (status == 0 && ncand > PTEFIT_MAX_CAND) status = 4;
   // 3. limiter vertices: bilinear flux, valid iff not behind any candidate as seen from the axis
@@ -160,6 +185,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
   }
   lm = block_argmax(lm, sh_am);
+  PTEFIT_SP(11);
   // 4. boundary flux
   double Pb = 0.0;
   if (status == 0) {
@@ -185,11 +211,15 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
     if (Pb == Pa) status = 1;
   }
+  PTEFIT_SP(12);
   // 5./6. plasma region and normalised flux
   int cnt = 0;
   if (status == 0) {
     const double inv = 1.0 / (Pb - Pa);
     int j = tid / nr, i = tid - j * nr;
+    T pco[2 * (PTEFIT_MAX_DEG + 1)];                   // registers: the stores below may alias o.pc for the compiler
+#pragma unroll
+    for (int k = 0; k < 2 * (PTEFIT_MAX_DEG + 1); ++k) pco[k] = o.pc ? o.pc[k] : T(0);
     for (int n = tid; n < N; n += nth) {
       T out = T(-1);
       const bool lmk = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
@@ -209,11 +239,11 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
       if (o.local) {
         T lv = out;
         if (o.pc) {                                   // I'(x) by Horner (fused_solve.cuh, delz column)
-          T hp = o.pc[PTEFIT_MAX_DEG], hq = o.pc[2 * PTEFIT_MAX_DEG + 1];
+          T hp = pco[PTEFIT_MAX_DEG], hq = pco[2 * PTEFIT_MAX_DEG + 1];
 #pragma unroll
           for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) {
-            hp = fma(hp, out, o.pc[k]);
-            hq = fma(hq, out, o.pc[PTEFIT_MAX_DEG + 1 + k]);
+            hp = fma(hp, out, pco[k]);
+            hq = fma(hq, out, pco[PTEFIT_MAX_DEG + 1 + k]);
           }
           lv = (out < T(0)) ? T(0) : fma(o.rdA[i], hp, o.fdA[i] * hq);
         }
@@ -230,6 +260,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   }
   if (cnt) atomicAdd(&sh_count, cnt);
   __syncthreads();
+  PTEFIT_SP(13);
   if (status == 0 && sh_count == 0) status = 1;
   if (tid == 0) {
     if (D.status[s] == 0) {
