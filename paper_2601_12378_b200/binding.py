@@ -260,3 +260,13 @@ class Reconstructor:
             self.close()
         except Exception:
             pass
+
+
+def shard_slices(n_slices, rank, world):
+    """Contiguous block of time slices rank `rank` of `world` reconstructs (slices are independent,
+    tables are replicated, no data-path collective).  Returns (first, count); earlier ranks take
+    the remainder."""
+    base, rem = divmod(int(n_slices), int(world))
+    count = base + (1 if rank < rem else 0)
+    first = rank * base + min(rank, rem)
+    return first, count
