@@ -126,58 +126,73 @@ __global__ void __launch_bounds__(RESP_THREADS) k_response(Dev<T> D) {
 // A4: least squares by normal equations + Cholesky in FP64 registers, column
 // equilibration and Tikhonov term per DESIGN.md reading O5.  One warp per slice.
 // grid ceil(B/4), block 128.
-template <typename T>
-__global__ void k_lsq(Dev<T> D, int B) {
+template <typename T, int NT>
+__global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
   const int s = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (s >= B) return;
-  const int nt = D.nt;
+  constexpr int nt = NT;                       // compile-time so that A, g, X stay in registers
   const T *resp = D.resp + (size_t)s * D.M * nt;
   const T *d = D.dred + (size_t)s * D.M;
-  constexpr int NA = PTEFIT_MAX_TERMS * (PTEFIT_MAX_TERMS + 1) / 2;
-  double A[NA], g[PTEFIT_MAX_TERMS];
+  constexpr int NA = NT * (NT + 1) / 2;
+  double A[NA], g[NT];
+#pragma unroll
   for (int k = 0; k < NA; ++k) A[k] = 0.0;
-  for (int k = 0; k < PTEFIT_MAX_TERMS; ++k) g[k] = 0.0;
+#pragma unroll
+  for (int k = 0; k < NT; ++k) g[k] = 0.0;
   bool finite = true;
   for (int m = lane; m < D.M; m += 32) {
     const double w = D.inv_sigma[m];
     const double y = (double)d[m] * w;
-    double r[PTEFIT_MAX_TERMS];
+    double r[NT];
+    #pragma unroll
     for (int l = 0; l < nt; ++l) { r[l] = (double)resp[m * nt + l] * w; finite &= isfinite(r[l]); }
     finite &= isfinite(y);
     int k = 0;
+    #pragma unroll
     for (int l = 0; l < nt; ++l) {
       g[l] = fma(r[l], y, g[l]);
+      #pragma unroll
       for (int q = 0; q <= l; ++q, ++k) A[k] = fma(r[l], r[q], A[k]);
     }
   }
   const int na = nt * (nt + 1) / 2;
+  #pragma unroll
   for (int k = 0; k < na; ++k) A[k] = warp_sum(A[k]);
+  #pragma unroll
   for (int l = 0; l < nt; ++l) g[l] = warp_sum(g[l]);
   finite = __all_sync(0xffffffffu, finite);
-  double X[PTEFIT_MAX_TERMS];
+  double X[NT];
   int st = 0;
   // every lane runs the tiny factorisation redundantly (no divergence, no broadcast needed)
-  double sc[PTEFIT_MAX_TERMS];
+  double sc[NT];
   bool any = false;
+  #pragma unroll
   for (int l = 0; l < nt; ++l) { sc[l] = sqrt(A[l * (l + 1) / 2 + l]); any |= sc[l] > 0.0; }
   if (!finite) st = 2; else if (!any) st = 3;
   const double reg = D.lambda_reg * D.lambda_reg * (double)D.M;
   // scaled matrix (unit diagonal + reg); dropped columns (sc = 0) become identity rows
   {
     int k = 0;
+    #pragma unroll
     for (int l = 0; l < nt; ++l)
+      #pragma unroll
       for (int q = 0; q <= l; ++q, ++k) {
         if (sc[l] > 0.0 && sc[q] > 0.0) A[k] = A[k] / (sc[l] * sc[q]) + (l == q ? reg : 0.0);
         else A[k] = (l == q) ? 1.0 : 0.0;
       }
+    #pragma unroll
     for (int l = 0; l < nt; ++l) g[l] = sc[l] > 0.0 ? g[l] / sc[l] : 0.0;
   }
   // Cholesky A = L L^T in place (row-packed lower triangle)
   double first_piv = 0.0;
-  for (int l = 0; l < nt && st == 0; ++l) {
+  #pragma unroll
+  for (int l = 0; l < nt; ++l) {
+    if (st != 0) break;
+    #pragma unroll
     for (int q = 0; q <= l; ++q) {
       double v = A[l * (l + 1) / 2 + q];
+      #pragma unroll
       for (int p = 0; p < q; ++p) v -= A[l * (l + 1) / 2 + p] * A[q * (q + 1) / 2 + p];
       if (q == l) {
         if (l == 0) first_piv = v;
@@ -188,24 +203,31 @@ __global__ void k_lsq(Dev<T> D, int B) {
       }
     }
   }
+  #pragma unroll
   for (int l = 0; l < nt; ++l) X[l] = 0.0;
   if (st == 0) {
+    #pragma unroll
     for (int l = 0; l < nt; ++l) {           // L z = g
       double v = g[l];
+      #pragma unroll
       for (int p = 0; p < l; ++p) v -= A[l * (l + 1) / 2 + p] * X[p];
       X[l] = v / A[l * (l + 1) / 2 + l];
     }
+    #pragma unroll
     for (int l = nt - 1; l >= 0; --l) {      // L^T x = z
       double v = X[l];
+      #pragma unroll
       for (int p = l + 1; p < nt; ++p) v -= A[p * (p + 1) / 2 + l] * X[p];
       X[l] = v / A[l * (l + 1) / 2 + l];
     }
+    #pragma unroll
     for (int l = 0; l < nt; ++l) X[l] = sc[l] > 0.0 ? X[l] / sc[l] : 0.0;
   }
   // chi^2 over the measurement rows
   double c2 = 0.0;
   for (int m = lane; m < D.M; m += 32) {
     double rsum = -(double)d[m];
+    #pragma unroll
     for (int l = 0; l < nt; ++l) rsum = fma((double)resp[m * nt + l], X[l], rsum);
     rsum *= D.inv_sigma[m];
     c2 = fma(rsum, rsum, c2);
@@ -214,6 +236,7 @@ __global__ void k_lsq(Dev<T> D, int B) {
   if (lane == 0) {
     const bool dead = D.status[s] != 0;       // status is sticky: a failed slice keeps its outputs
     if (!dead) {
+      #pragma unroll
       for (int l = 0; l < nt; ++l) { D.Xprev[(size_t)s * nt + l] = D.X[(size_t)s * nt + l]; D.X[(size_t)s * nt + l] = X[l]; }
       D.chi2[s] = c2;
       if (st != 0) D.status[s] = st;

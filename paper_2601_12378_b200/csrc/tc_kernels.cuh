@@ -71,11 +71,35 @@ __global__ void k_resp_reduce(Dev<float> D, TcDev Tc) {
   D.resp[((size_t)s * D.M + m) * D.nt + l] = acc;
 }
 
-// Node currents on the compact list, split for 3xTF32.  grid (Kc/256, B), block 256.
-__global__ void k_cur_split(Dev<float> D, TcDev Tc) {
+// A5 on the compact node list: I = J_b X by Horner evaluation of the per-slice
+// polynomials rdA P(x) + fdA Q(x) (+ delz column), written to cur[s][n] (for the Delta* solve; nodes
+// outside the list stay zero) and, split for 3xTF32, to cur_hi/lo[s][kc].  grid (Kc/256, B), block 256.
+__global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
+  __shared__ float pco[2 * (PTEFIT_MAX_DEG + 1)];
+  __shared__ float xdz;
   const int s = blockIdx.y, kc = blockIdx.x * blockDim.x + threadIdx.x;
+  const double *X = D.X + (size_t)s * D.nt;
+  if (threadIdx.x < 2 * (PTEFIT_MAX_DEG + 1)) {
+    const int kind = threadIdx.x / (PTEFIT_MAX_DEG + 1), k = threadIdx.x - kind * (PTEFIT_MAX_DEG + 1);
+    double c = 0.0;
+    for (int l = 0; l < D.npoly; ++l)
+      if (D.terms[l].kind == kind) c += X[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+    pco[threadIdx.x] = float(c);
+  }
+  if (threadIdx.x == 32) xdz = D.has_delz ? float(X[D.nt - 1]) : 0.f;
+  __syncthreads();
   if (kc >= Tc.Kc) return;
-  const float v = D.cur[(size_t)s * D.N + Tc.cnode[kc]];
+  const int n = Tc.cnode[kc];
+  const float x = D.xn[(size_t)s * D.N + n];
+  const int i = n % D.nr;
+  const float R = float(D.rmin + i * D.dr);
+  const float rdA = R * float(D.dA), fdA = float(kMu0 * D.dA) / R;
+  float hp = pco[PTEFIT_MAX_DEG], hq = pco[2 * PTEFIT_MAX_DEG + 1];
+#pragma unroll
+  for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fmaf(hp, x, pco[k]); hq = fmaf(hq, x, pco[PTEFIT_MAX_DEG + 1 + k]); }
+  float v = (x < 0.f) ? 0.f : fmaf(rdA, hp, fdA * hq);
+  if (D.has_delz) v = fmaf(D.dzc[(size_t)s * D.N + n], xdz, v);
+  if (n != 0) D.cur[(size_t)s * D.N + n] = v;        // padding entries point at node 0
   const float hi = tf32_rna(v);
   Tc.cur_hi[(size_t)s * Tc.Kc + kc] = hi;
   Tc.cur_lo[(size_t)s * Tc.Kc + kc] = tf32_rna(v - hi);
