@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
                                                                 int do_search) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nr = D.nr, nz = D.nz, N = D.N, nri = D.nri, nzi = D.nzi, Nz = nz - 1, n2 = Nz / 2;
-  const int tid = threadIdx.x, nth = blockDim.x;
+  const int tid = threadIdx.x, nth = blockDim.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
   T *G = reinterpret_cast<T *>(smem_raw);
   T *So = G + ((N + 3) & ~3);
   T *Se = So + n2 * n2;
@@ -187,24 +187,25 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     __syncthreads();
     PTEFIT_PHASE(15);
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
-    {
-      int j = tid / nr, i = tid - j * nr;
-      for (int n = tid; n < N; n += nth) {
-        T v;
-        if (j == 0) v = pb[i];
-        else if (j == nz - 1) v = pb[nr + i];
-        else if (i == 0) v = pb[2 * nr + j - 1];
-        else if (i == nr - 1) v = pb[2 * nr + nzi + j - 1];
-        else {
-          v = c_rhs[i] * G[n];
-          if (i == 1) v -= c_edge[0] * pb[2 * nr + j - 1];
-          if (i == nri) v -= c_edge[1] * pb[2 * nr + nzi + j - 1];
-          if (j == 1) v -= cz * pb[i];
-          if (j == nzi) v -= cz * pb[nr + i];
-        }
-        G[n] = v;
-        i += nth;
-        while (i >= nr) { i -= nr; ++j; }
+    // (one warp per grid row: the row tests are warp-uniform, the column tests plain selects)
+    for (int j = warp; j < nz; j += nwarp) {
+      T *row = G + j * nr;
+      if (j == 0 || j == nz - 1) {
+        const T *src = pb + (j ? nr : 0);
+        for (int i = lane; i < nr; i += 32) row[i] = src[i];
+        continue;
+      }
+      const T pl = pb[2 * nr + j - 1], pr = pb[2 * nr + nzi + j - 1];
+      const T el = c_edge[0] * pl, er = c_edge[1] * pr;
+      for (int i = lane; i < nr; i += 32) {
+        T v = c_rhs[i] * row[i];
+        if (i == 1) v -= el;
+        if (i == nri) v -= er;
+        if (j == 1) v -= cz * pb[i];
+        if (j == nzi) v -= cz * pb[nr + i];
+        if (i == 0) v = pl;
+        if (i == nr - 1) v = pr;
+        row[i] = v;
       }
     }
     __syncthreads();
@@ -266,42 +267,43 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     SearchOpt<T> so_opt;
     so_opt.am.v = -INFINITY; so_opt.am.n = 0x7fffffff;
     {
-      constexpr int EB = 8;
-      int j = tid / nr, i = tid - j * nr;
-      T cn[EB], on[EB];                                    // next batch, in flight while this one is used
+      // one warp per grid row; the global loads of a row (and of the next row) are in flight
+      // before they are used
+      constexpr int KR = (PTEFIT_MAX_NR + 31) / 32;
+      auto load_row = [&](int j, T *cv, T *ov) {
 #pragma unroll
-      for (int u = 0; u < EB; ++u) {
-        const int n = tid + u * nth;
-        cn[u] = (add_coil && n < N) ? pc[n] : T(0);
-        on[u] = (use_relax && n < N) ? psi[n] : T(0);
-      }
-      for (int n0 = tid; n0 < N; n0 += EB * nth) {
-        T cv[EB], ov[EB];
-#pragma unroll
-        for (int u = 0; u < EB; ++u) { cv[u] = cn[u]; ov[u] = on[u]; }
-#pragma unroll
-        for (int u = 0; u < EB; ++u) {
-          const int n = n0 + (EB + u) * nth;
-          cn[u] = (add_coil && n < N) ? pc[n] : T(0);
-          on[u] = (use_relax && n < N) ? psi[n] : T(0);
+        for (int k = 0; k < KR; ++k) {
+          const int i = lane + 32 * k;
+          const bool ok = (j < nz) && (i < nr);
+          cv[k] = (add_coil && ok) ? pc[j * nr + i] : T(0);
+          ov[k] = (use_relax && ok) ? psi[j * nr + i] : T(0);
         }
+      };
+      T cn[KR], on[KR];
+      load_row(warp, cn, on);
+      for (int j = warp; j < nz; j += nwarp) {
+        T cv[KR], ov[KR];
 #pragma unroll
-        for (int u = 0; u < EB; ++u) {
-          const int n = n0 + u * nth;
-          if (n < N) {
-            const bool edge = (j == 0) | (j == nz - 1) | (i == 0) | (i == nr - 1);
-            T v = edge ? G[n] : G[n] * scale;
-            v += cv[u];
-            if (use_relax) v = ov[u] + om * (v - ov[u]);
-            psi[n] = v;
-            G[n] = v;
+        for (int k = 0; k < KR; ++k) { cv[k] = cn[k]; ov[k] = on[k]; }
+        load_row(j + nwarp, cn, on);
+        const bool erow = (j == 0) | (j == nz - 1);
+        T *row = G + j * nr;
+#pragma unroll
+        for (int k = 0; k < KR; ++k) {
+          const int i = lane + 32 * k;
+          if (i < nr) {
+            const bool edge = erow | (i == 0) | (i == nr - 1);
+            T v = edge ? row[i] : row[i] * scale;
+            v += cv[k];
+            if (use_relax) v = ov[k] + om * (v - ov[k]);
+            psi[j * nr + i] = v;
+            row[i] = v;
             if (do_search) {
+              const int n = j * nr + i;
               const double dv = (double)v;
               so_opt.bad |= !isfinite(dv);
               if ((mbits[n >> 5] >> (n & 31)) & 1u) { ArgMax c; c.v = sg * dv; c.n = n; so_opt.am = better(so_opt.am, c); }
             }
-            i += nth;
-            while (i >= nr) { i -= nr; ++j; }
           }
         }
       }
@@ -320,13 +322,14 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
         __syncthreads();
         T *dzc = D.dzc + (size_t)s * N;
         const T hz = T(0.5 / D.dz);
-        int j = tid / nr, i = tid - j * nr;
-        for (int n = tid; n < N; n += nth) {
-          T out = T(0);
-          if (j >= 1 && j <= nz - 2 && i >= 1 && i <= nr - 2) out = -(G[n + nr] - G[n - nr]) * hz;
-          dzc[n] = out;
-          i += nth;
-          while (i >= nr) { i -= nr; ++j; }
+        for (int j = warp; j < nz; j += nwarp) {
+          const bool irow = (j >= 1) & (j <= nz - 2);
+          const T *row = G + j * nr;
+          for (int i = lane; i < nr; i += 32) {
+            T out = T(0);
+            if (irow && i >= 1 && i <= nr - 2) out = -(row[i + nr] - row[i - nr]) * hz;
+            dzc[j * nr + i] = out;
+          }
         }
       }
       PTEFIT_PHASE(6);

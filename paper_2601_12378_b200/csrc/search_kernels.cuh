@@ -86,8 +86,8 @@ struct SearchOpt {
 
 template <typename T>
 __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, const SearchOpt<T> &o) {
-  const int nth = blockDim.x, tid = threadIdx.x;
-  const int nr = D.nr, N = D.N;
+  const int nth = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
+  const int nr = D.nr, nz = D.nz, N = D.N;
   const double sg = (double)D.ip_sign;
   __shared__ ArgMax sh_am[32];
   __shared__ int sh_flag, sh_ncand, sh_count;
@@ -102,12 +102,14 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   bool bad = false;
   if (o.have_am) { am = o.am; bad = o.bad; }
   else {
-    for (int n = tid; n < N; n += nth) {
-      const double v = (double)psi[n];
-      bad |= !isfinite(v);
-      const bool lm = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
-      if (lm) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
-    }
+    for (int j = warp; j < nz; j += nwarp)
+      for (int i = lane; i < nr; i += 32) {
+        const int n = j * nr + i;
+        const double v = (double)psi[n];
+        bad |= !isfinite(v);
+        const bool lm = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
+        if (lm) { ArgMax c; c.v = sg * v; c.n = n; am = better(am, c); }
+      }
   }
   if (bad) atomicOr(&sh_flag, 1);
   am = block_argmax(am, sh_am);
@@ -125,7 +127,10 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   PTEFIT_SP(9);
   // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
   if (status == 0) {
-    for (int n = tid; n < N; n += nth) {
+    for (int j = warp + 1; j < nz - 1; j += nwarp)
+     for (int i = lane; i < nr - 1; i += 32) {
+      if (i == 0) continue;
+      const int n = j * nr + i;
       const bool xm = o.xbits ? ((o.xbits[n >> 5] >> (n & 31)) & 1u) : D.xpt_mask[n];
       if (!xm) continue;
       if (sizeof(T) == 4) {
@@ -156,7 +161,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
       if (f.det < 0.0 && fabs(f.xs) <= 0.5 && fabs(f.ys) <= 0.5 && sg * f.ps < sg * Pa) {
         const int q = atomicAdd(&sh_ncand, 1);
         if (q < PTEFIT_MAX_CAND) {
-          const int j = n / nr, i = n - j * nr;
           cR[q] = D.rmin + (i + f.xs) * D.dr; cZ[q] = D.zmin + (j + f.ys) * D.dz; cP[q] = f.ps; cN[q] = n;
         }
       }
@@ -216,11 +220,12 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   int cnt = 0;
   if (status == 0) {
     const double inv = 1.0 / (Pb - Pa);
-    int j = tid / nr, i = tid - j * nr;
     T pco[2 * (PTEFIT_MAX_DEG + 1)];                   // registers: the stores below may alias o.pc for the compiler
 #pragma unroll
     for (int k = 0; k < 2 * (PTEFIT_MAX_DEG + 1); ++k) pco[k] = o.pc ? o.pc[k] : T(0);
-    for (int n = tid; n < N; n += nth) {
+    for (int j = warp; j < nz; j += nwarp)
+     for (int i = lane; i < nr; i += 32) {
+      const int n = j * nr + i;
       T out = T(-1);
       const bool lmk = o.lbits ? ((o.lbits[n >> 5] >> (n & 31)) & 1u) : D.lim_mask[n];
       if (lmk) {
@@ -249,8 +254,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
         }
         o.local[n] = lv;
       }
-      i += nth;
-      while (i >= nr) { i -= nr; ++j; }
     }
   } else {
     for (int n = tid; n < N; n += nth) {
