@@ -36,6 +36,8 @@ struct ptefit_handle {
   TcDev Tc{};
   const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;
   int pbd_ntiles = 0;
+  const float *c_rdA = nullptr, *c_fdA = nullptr;   // Eq. 10 factors on the compact node list
+  int std_np = 0;                       // > 0: standard term list, basis generated inside the response GEMM
   CUtensorMap mapJbHi, mapJbLo, mapGpHi, mapGpLo, mapCurHi, mapCurLo, mapGbHi, mapGbLo;
   long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)

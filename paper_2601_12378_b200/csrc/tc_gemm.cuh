@@ -123,11 +123,23 @@ struct GemmSmem {
 // finished chunk into FP32 registers (round-to-nearest) while the next chunk is being multiplied.
 // grid (M tiles, N tiles, splits), block GEMM_THREADS, dyn smem GemmSmem<BN,STAGES>::BYTES.
 // out: [splits][m_rows][ldo] floats, m_rows = gridDim.x * BM, ldo >= gridDim.y * BN.
-template <int BN, int STAGES>
-__global__ void __launch_bounds__(GEMM_THREADS, 1)
+// With NP > 0 the A operand (basis columns of Eq. 10, for the standard term list
+// NP P' terms x^i - x^NP, NFF FF' terms x^j - x^NFF, optional delz column; 8 rows per slice) is
+// generated by four producer warps straight into the swizzled shared-memory tiles instead of
+// being loaded by TMA: J_b is never materialised in HBM.
+struct AProd {
+  const float *xn, *dzc;      // [B][N] normalised flux (-1 outside the mask), delz column
+  const int *cnode;           // [Kc] compact node list
+  const float *rdA, *fdA;     // [Kc] R dA and mu0 dA / R of the compact nodes
+  int N, B, has_delz;
+};
+template <int NP> constexpr int gemm_threads() { return NP > 0 ? 448 : GEMM_THREADS; }
+
+template <int BN, int STAGES, int NP = 0, int NFF = 0>
+__global__ void __launch_bounds__(gemm_threads<NP>(), 1)
 k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant__ CUtensorMap mapAlo,
               const __grid_constant__ CUtensorMap mapBhi, const __grid_constant__ CUtensorMap mapBlo,
-              float *__restrict__ out, int ldo, int kblocks) {
+              float *__restrict__ out, int ldo, int kblocks, const AProd ap) {
   using L = GemmSmem<BN, STAGES>;
   static_assert(BN % 16 == 0 && BN <= 256, "N tile");
   extern __shared__ unsigned char smem_raw[];
@@ -147,9 +159,16 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&mapAhi); tma_prefetch_desc(&mapAlo); tma_prefetch_desc(&mapBhi); tma_prefetch_desc(&mapBlo);
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, NP > 0 ? 5 : 1); mbar_init(empty + s, 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 8); }
     fence_barrier_init();
+  }
+  if (NP > 0) {                                        // rows of unused terms stay zero for the whole kernel
+    for (int e = threadIdx.x; e < STAGES * 2 * L::A_BYTES / 16; e += blockDim.x) {
+      const int st = e / (2 * L::A_BYTES / 16), w = e - st * (2 * L::A_BYTES / 16);
+      reinterpret_cast<uint4 *>(base + st * L::STAGE_BYTES)[w] = make_uint4(0, 0, 0, 0);
+    }
+    fence_proxy_async();
   }
   if (warp == 1) tmem_alloc<TMEM_COLS>(tmem_slot);
   tc_fence_before();
@@ -164,9 +183,11 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
         mbar_wait(empty + s, ph ^ 1u);
         unsigned char *st = base + s * L::STAGE_BYTES;
-        mbar_expect_tx(full + s, (uint32_t)L::STAGE_BYTES);
-        tma_load_2d(st, &mapAhi, full + s, kb * BK, m0);
-        tma_load_2d(st + L::A_BYTES, &mapAlo, full + s, kb * BK, m0);
+        mbar_expect_tx(full + s, (uint32_t)(NP > 0 ? 2 * L::B_BYTES : L::STAGE_BYTES));
+        if (NP == 0) {
+          tma_load_2d(st, &mapAhi, full + s, kb * BK, m0);
+          tma_load_2d(st + L::A_BYTES, &mapAlo, full + s, kb * BK, m0);
+        }
         tma_load_2d(st + 2 * L::A_BYTES, &mapBhi, full + s, kb * BK, n0);
         tma_load_2d(st + 2 * L::A_BYTES + L::B_BYTES, &mapBlo, full + s, kb * BK, n0);
       }
@@ -202,7 +223,65 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         tc_commit(tfull + buf);                        // chunk complete
       }
     }
-  } else {                                             // ---- promotion to registers + epilogue
+  } else if (NP > 0 && warp >= 10) {                   // ---- basis producers (warps 10-13)
+    constexpr int NPOLY = NP + NFF;
+    constexpr int PMAX = NP > NFF ? NP : NFF;
+    const int pw_ = warp - 10;                          // handles slices 4 pw_ .. 4 pw_ + 3 of the tile
+    const int sbase = m0 / 8 + 4 * pw_;
+    float xv[4], dv[4], rd, fd;
+    auto fetch = [&](int kb, float *x, float *d, float &r, float &f) {
+      const int kc = kb * BK + lane;
+      const int n = ap.cnode[kc];
+      r = ap.rdA[kc]; f = ap.fdA[kc];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int sl = min(sbase + q, ap.B - 1);
+        x[q] = ap.xn[(size_t)sl * ap.N + n];
+        d[q] = ap.has_delz ? ap.dzc[(size_t)sl * ap.N + n] : 0.f;
+      }
+    };
+    if (kb0 < kb1) fetch(kb0, xv, dv, rd, fd);
+    for (int kb = kb0, it = 0; kb < kb1; ++kb, ++it) {
+      const int s = it % STAGES;
+      const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
+      float x[4], d[4];
+      const float r = rd, f = fd;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) { x[q] = xv[q]; d[q] = dv[q]; }
+      if (kb + 1 < kb1) fetch(kb + 1, xv, dv, rd, fd);   // next block's loads fly during this block's math
+      mbar_wait(empty + s, ph ^ 1u);
+      unsigned char *ahi = base + s * L::STAGE_BYTES, *alo = ahi + L::A_BYTES;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        float pwv[PMAX + 1];
+        pwv[0] = 1.f;
+#pragma unroll
+        for (int k = 1; k <= PMAX; ++k) pwv[k] = pwv[k - 1] * x[q];
+        const bool in = !(x[q] < 0.f);
+        const uint32_t rowbase = (uint32_t)(4 * pw_ + q) * 1024u + (uint32_t)(lane & 3) * 4u;
+#pragma unroll
+        for (int l = 0; l < NPOLY + 1; ++l) {
+          float v;
+          if (l < NP) v = in ? (pwv[l] - pwv[NP]) * r : 0.f;
+          else if (l < NPOLY) v = in ? (pwv[l - NP] - pwv[NFF]) * f : 0.f;
+          else v = d[q];
+          if (l == NPOLY && !ap.has_delz) break;
+          const float hi = __uint_as_float(__float_as_uint(v));
+          uint32_t hr;
+          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(hr) : "f"(hi));
+          const float hf = __uint_as_float(hr);
+          uint32_t lr;
+          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(lr) : "f"(v - hf));
+          const uint32_t off = rowbase + (uint32_t)l * 128u + ((((uint32_t)lane >> 2) ^ (uint32_t)l) << 4);
+          *reinterpret_cast<uint32_t *>(ahi + off) = hr;
+          *reinterpret_cast<uint32_t *>(alo + off) = lr;
+        }
+      }
+      fence_proxy_async();                              // generic-proxy writes -> visible to tcgen05.mma
+      __syncwarp();
+      if (lane == 0) mbar_arrive(full + s);
+    }
+  } else if (warp >= 2 && warp < 10) {                 // ---- promotion to registers + epilogue
     const int q = warp & 3;                            // TMEM lane quarter this warp may access
     const int half = (warp - 2) >> 2;                  // which half of the columns
     constexpr int C0 = ((BN / 16 + 1) / 2) * 16;       // columns of half 0 (multiple of 16)
