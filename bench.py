@@ -270,7 +270,12 @@ def run_ours(args):
     peaks = _peaks()
     roof = stage_roofline(top, loop_stages[top] / n_iter, dims, peaks, args.gemm)
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None                          # filled from profiles/ (ncu --set full) in DESIGN.md
+    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the committed
+    # `ncu --set full` capture of this workload, profiles/r1_v9_ncu_full.md; null for other workloads
+    ncu_traffic = {"k_solve_fused": 216.7e6, "response": 54.1e6, "boundary": 65.8e6}
+    roof["traffic"] = None
+    if args.config == "cfg4" and B == 512:
+        roof["traffic"] = ncu_traffic.get("k_solve_fused" if top == "solve" else top)
     roof["share_of_step"] = loop_stages[top] / max(sum(acc.values()), 1e-9)
     roof["all_stages"] = {}
     for sname, ms in loop_stages.items():
