@@ -35,6 +35,7 @@ struct Dev {
   TermDev terms[PTEFIT_MAX_TERMS];
   // tables (device)
   const T *gp, *gc, *gb, *ggc;
+  const T *ggc_t;                 // ggc transposed: [n_c][N]
   const double *inv_sigma;        // [M]
   const uint8_t *lim_mask, *xpt_mask;
   const unsigned *lim_bits, *xpt_bits;   // the same masks bit-packed: bit (n & 31) of word n >> 5

@@ -17,9 +17,10 @@ __global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__
   __syncthreads();
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n < D.N) {
-    const T *g = D.ggc + (size_t)n * D.nc;
+    const T *g = D.ggc_t + n;                       // transposed table [n_c][N]: coalesced over nodes
     T acc = T(0);
-    for (int c = 0; c < D.nc; ++c) acc = fma(g[c], sic[c], acc);
+#pragma unroll 4
+    for (int c = 0; c < D.nc; ++c) acc = fma(g[(size_t)c * D.N], sic[c], acc);
     D.psi_coil[(size_t)s * D.N + n] = acc;
   }
   if (n < D.M) {

@@ -131,6 +131,12 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   TRY(upload(h, &D.gc, tb->gc, (size_t)D.M * D.nc));
   TRY(upload(h, &D.ggc, tb->ggc, N * D.nc));
   {
+    std::vector<double> t((size_t)D.nc * N);
+    for (size_t n = 0; n < N; ++n)
+      for (int c = 0; c < D.nc; ++c) t[(size_t)c * N + n] = tb->ggc[n * D.nc + c];
+    TRY(upload(h, &D.ggc_t, t.data(), t.size()));
+  }
+  {
     std::vector<double> w(D.M);
     for (int m = 0; m < D.M; ++m) w[m] = 1.0 / ge->sigma[m];
     TRY(upload(h, &D.inv_sigma, w.data(), w.size()));

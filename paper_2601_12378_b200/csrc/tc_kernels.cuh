@@ -15,6 +15,7 @@ struct TcDev {
   int rows_resp, rows_pbd;  // padded row counts (multiples of 128)
   int split_resp, split_pbd;
   const int *cnode;       // [Kc]
+  const float *rdA, *fdA; // [Kc] R dA and mu0 dA / R of the compact nodes (Eq. 10 factors)
   float *jb_hi, *jb_lo;   // [rows_resp][Kc]
   float *cur_hi, *cur_lo; // [rows_pbd][Kc]
   float *resp_part;       // [split_resp][rows_resp][ld_resp]
@@ -73,11 +74,11 @@ __global__ void k_resp_reduce(Dev<float> D, TcDev Tc) {
 
 // A5 on the compact node list: I = J_b X by Horner evaluation of the per-slice
 // polynomials rdA P(x) + fdA Q(x) (+ delz column), written to cur[s][n] (for the Delta* solve; nodes
-// outside the list stay zero) and, split for 3xTF32, to cur_hi/lo[s][kc].  grid (Kc/256, B), block 256.
+// outside the list stay zero) and, split for 3xTF32, to cur_hi/lo[s][kc].  grid (Kc/1024, B), block 256.
 __global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
   __shared__ float pco[2 * (PTEFIT_MAX_DEG + 1)];
   __shared__ float xdz;
-  const int s = blockIdx.y, kc = blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = blockIdx.y;
   const double *X = D.X + (size_t)s * D.nt;
   if (threadIdx.x < 2 * (PTEFIT_MAX_DEG + 1)) {
     const int kind = threadIdx.x / (PTEFIT_MAX_DEG + 1), k = threadIdx.x - kind * (PTEFIT_MAX_DEG + 1);
@@ -88,21 +89,27 @@ __global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
   }
   if (threadIdx.x == 32) xdz = D.has_delz ? float(X[D.nt - 1]) : 0.f;
   __syncthreads();
-  if (kc >= Tc.Kc) return;
-  const int n = Tc.cnode[kc];
-  const float x = D.xn[(size_t)s * D.N + n];
-  const int i = n % D.nr;
-  const float R = float(D.rmin + i * D.dr);
-  const float rdA = R * float(D.dA), fdA = float(kMu0 * D.dA) / R;
-  float hp = pco[PTEFIT_MAX_DEG], hq = pco[2 * PTEFIT_MAX_DEG + 1];
+  float cp[2 * (PTEFIT_MAX_DEG + 1)];
 #pragma unroll
-  for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fmaf(hp, x, pco[k]); hq = fmaf(hq, x, pco[PTEFIT_MAX_DEG + 1 + k]); }
-  float v = (x < 0.f) ? 0.f : fmaf(rdA, hp, fdA * hq);
-  if (D.has_delz) v = fmaf(D.dzc[(size_t)s * D.N + n], xdz, v);
-  if (n != 0) D.cur[(size_t)s * D.N + n] = v;        // padding entries point at node 0
-  const float hi = tf32_rna(v);
-  Tc.cur_hi[(size_t)s * Tc.Kc + kc] = hi;
-  Tc.cur_lo[(size_t)s * Tc.Kc + kc] = tf32_rna(v - hi);
+  for (int k = 0; k < 2 * (PTEFIT_MAX_DEG + 1); ++k) cp[k] = pco[k];
+  const float xd = xdz;
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int kq = (blockIdx.x * 4 + u) * blockDim.x + threadIdx.x;
+    if (kq >= Tc.Kc) continue;
+    const int n = Tc.cnode[kq];
+    const float x = D.xn[(size_t)s * D.N + n];
+    const float rdA = Tc.rdA[kq], fdA = Tc.fdA[kq];
+    float hp = cp[PTEFIT_MAX_DEG], hq = cp[2 * PTEFIT_MAX_DEG + 1];
+#pragma unroll
+    for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fmaf(hp, x, cp[k]); hq = fmaf(hq, x, cp[PTEFIT_MAX_DEG + 1 + k]); }
+    float v = (x < 0.f) ? 0.f : fmaf(rdA, hp, fdA * hq);
+    if (D.has_delz) v = fmaf(D.dzc[(size_t)s * D.N + n], xd, v);
+    if (n != 0) D.cur[(size_t)s * D.N + n] = v;        // padding entries point at node 0
+    const float hi = tf32_rna(v);
+    Tc.cur_hi[(size_t)s * Tc.Kc + kq] = hi;
+    Tc.cur_lo[(size_t)s * Tc.Kc + kq] = tf32_rna(v - hi);
+  }
 }
 
 // psi_bdry[s][k] = sum_z pbd_part[z][s][k].  grid (ceil(nbnd/256), B).
