@@ -43,6 +43,8 @@ struct Dev {
   // Delta* solve factors: [nri][nzi] (i-major so that threads over m coalesce)
   const double *tri_w, *tri_invb; // Thomas multipliers and inverse pivots
   const double *tri_ce;           // [nri] super-diagonal
+  const double *tw2, *tib2;       // [nri][nzi] twisted factorisation (two threads per mode), see ptefit.cu
+  const double *tw2k, *tod2;      // [nzi] right multiplier of the middle row; [nri] off-diagonals
   const T *sintab;                // [2*(nz-1)] sin(pi k/(nz-1))
   const T *dst_tab;               // folded DST matrices So[n2][n2], Se[n2][n2] (fused_solve.cuh)
   // workspaces [max_batch][...]

@@ -214,7 +214,66 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     PTEFIT_PHASE(1);
     // ---- Thomas sweeps along R in FP64, one thread per mode (precomputed factors).
     // The dependent chain is one DFMA per step.
-    if (tid < nzi) {
+    if (2 * nzi <= nth && nri >= 3) {
+      // twisted factorisation: threads [0, nth/2) eliminate rows 0..k-1 downwards, threads
+      // [nth/2, nth) rows n-1..k+1 upwards; row k couples the halves; both substitute outwards.
+      const int half = nth >> 1, side = tid >= half, mm = tid - side * half;
+      const int n = nri, k = n / 2, len = side ? n - 1 - k : k;
+      double *ex = reinterpret_cast<double *>(E);          // [2][half] elimination results next to row k
+      const bool act = mm < nzi;
+      T *row = G + (mm + 1) * nr + 1;
+      double *__restrict__ y = D.ytmp + (size_t)blockIdx.x * nri * nzi + mm;
+      const double *__restrict__ tw = D.tw2 + mm;
+      const double *__restrict__ tb = D.tib2 + mm;
+      const double *__restrict__ tod = D.tod2;
+      constexpr int U = 8;
+      double prev = 0.0;
+      if (act) {
+        for (int t0 = 0; t0 < len; t0 += U) {
+          double w[U];
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int t = t0 + u, i = side ? n - 1 - t : t;
+            w[u] = (t < len) ? __ldg(tw + (size_t)i * nzi) : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int t = t0 + u, i = side ? n - 1 - t : t;
+            if (t < len) {
+              const double v = fma(-w[u], prev, (double)row[i]);
+              y[(size_t)i * nzi] = v;
+              prev = v;
+            }
+          }
+        }
+        ex[side * half + mm] = prev;                       // y_{k-1} (left) or y_{k+1} (right)
+      }
+      __syncthreads();
+      double x = 0.0;
+      if (act) {
+        const double yk = (double)row[k] - __ldg(tw + (size_t)k * nzi) * ex[mm] - __ldg(D.tw2k + mm) * ex[half + mm];
+        x = yk * __ldg(tb + (size_t)k * nzi);
+        if (!side) row[k] = T(x);
+        for (int t0 = len - 1; t0 >= 0; t0 -= U) {
+          double a[U], b[U];
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int t = t0 - u, i = side ? n - 1 - t : t;
+            const double ib = t >= 0 ? __ldg(tb + (size_t)i * nzi) : 0.0;
+            a[u] = t >= 0 ? y[(size_t)i * nzi] * ib : 0.0;
+            b[u] = t >= 0 ? __ldg(tod + i) * ib : 0.0;
+          }
+#pragma unroll
+          for (int u = 0; u < U; ++u) {
+            const int t = t0 - u, i = side ? n - 1 - t : t;
+            if (t >= 0) {
+              x = fma(-b[u], x, a[u]);                     // x_i = (y_i - offdiag_i x_neighbour) / piv_i
+              row[i] = T(x);
+            }
+          }
+        }
+      }
+    } else     if (tid < nzi) {
       const int mm = tid;
       T *row = G + (mm + 1) * nr + 1;
       double *__restrict__ y = D.ytmp + (size_t)blockIdx.x * nri * nzi + mm;

@@ -182,6 +182,32 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
     TRY(upload(h, &D.tri_w, w.data(), w.size()));
     TRY(upload(h, &D.tri_invb, ib.data(), ib.size()));
     TRY(upload(h, &D.tri_ce, ce.data(), ce.size()));
+    // Twisted (two-sided) factorisation of the same systems for k_solve_fused: rows 0..k-1 are
+    // eliminated downwards, rows n-1..k+1 upwards, row k = n/2 couples both halves, so two threads
+    // per mode walk chains of half the length.  tw2[i][m]: multiplier of row i (towards the
+    // previous row of its half; row k: the left one), tw2k[m]: right multiplier of row k,
+    // tib2[i][m]: inverse pivots, tod2[i]: off-diagonal used in the back substitution of row i.
+    {
+      const int n = nri, k = n / 2;
+      std::vector<double> w2((size_t)n * nzi, 0.0), ib2((size_t)n * nzi, 0.0), wk(nzi, 0.0), od(n, 0.0);
+      for (int i = 0; i < n; ++i) od[i] = (i < k) ? ce[i] : cw[i];
+      for (int mm = 0; mm < nzi; ++mm) {
+        const double sn = sin(pi * (mm + 1) / (2.0 * (D.nz - 1)));
+        const double diag = -2.0 / (D.dr * D.dr) - 4.0 / (D.dz * D.dz) * sn * sn;
+        std::vector<double> piv(n, diag);
+        for (int i = 1; i < k; ++i) { const double wl = cw[i] / piv[i - 1]; w2[(size_t)i * nzi + mm] = wl; piv[i] = diag - wl * ce[i - 1]; }
+        for (int i = n - 2; i > k; --i) { const double wr = ce[i] / piv[i + 1]; w2[(size_t)i * nzi + mm] = wr; piv[i] = diag - wr * cw[i + 1]; }
+        double pk = diag;
+        if (k >= 1) { const double wl = cw[k] / piv[k - 1]; w2[(size_t)k * nzi + mm] = wl; pk -= wl * ce[k - 1]; }
+        if (k + 1 < n) { const double wr = ce[k] / piv[k + 1]; wk[mm] = wr; pk -= wr * cw[k + 1]; }
+        piv[k] = pk;
+        for (int i = 0; i < n; ++i) ib2[(size_t)i * nzi + mm] = 1.0 / piv[i];
+      }
+      TRY(upload(h, &D.tw2, w2.data(), w2.size()));
+      TRY(upload(h, &D.tib2, ib2.data(), ib2.size()));
+      TRY(upload(h, &D.tw2k, wk.data(), wk.size()));
+      TRY(upload(h, &D.tod2, od.data(), od.size()));
+    }
     const int period = 2 * (D.nz - 1);
     std::vector<double> st(period);
     for (int k = 0; k < period; ++k) st[k] = sin(pi * k / (D.nz - 1));
