@@ -55,8 +55,8 @@ __host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
 template <typename T>
 __device__ void dst_columns(T *G, const T *So, const T *Se, T *E, int nr, int nz) {
   const int Nz = nz - 1, n2 = Nz / 2, nri = nr - 2, nzi = nz - 2;
-  const int nq = n2 / 4, ncp = FUSED_CW / 2;
-  const int items = 2 * nq * ncp;
+  const int nq = n2 / 4, ncq = FUSED_CW / 4;
+  const int items = 2 * nq * ncq;                              // 4 modes x 4 columns per item
   const int tid = threadIdx.x, nth = blockDim.x;
   for (int c0 = 0; c0 < nri; c0 += FUSED_CW) {
     for (int e = tid; e < n2 * FUSED_CW; e += nth) {          // fold rows j and Nz-j
@@ -73,28 +73,29 @@ __device__ void dst_columns(T *G, const T *So, const T *Se, T *E, int nr, int nz
     }
     __syncthreads();
     for (int it = tid; it < items; it += nth) {
-      const int cp = it % ncp, q = (it / ncp) % nq, par = it / (ncp * nq);
+      const int cq = it % ncq, q = (it / ncq) % nq, par = it / (ncq * nq);
       const T *St = (par ? Se : So) + 4 * q;
-      const T *Ep = E + par * n2 * FUSED_CW + 2 * cp;
-      T acc[4][2];
+      const T *Ep = E + par * n2 * FUSED_CW + 4 * cq;
+      T acc[4][4];
 #pragma unroll
-      for (int r = 0; r < 4; ++r) acc[r][0] = acc[r][1] = T(0);
-#pragma unroll 8
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int t = 0; t < 4; ++t) acc[r][t] = T(0);
+#pragma unroll 4
       for (int j = 0; j < n2; ++j) {
         const Vec4<T> sv = load4(St + j * n2);
-        const Vec2<T> ev = load2(Ep + j * FUSED_CW);
+        const Vec4<T> ev = load4(Ep + j * FUSED_CW);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          acc[r][0] = fma(sv.v[r], ev.v[0], acc[r][0]);
-          acc[r][1] = fma(sv.v[r], ev.v[1], acc[r][1]);
-        }
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int t = 0; t < 4; ++t) acc[r][t] = fma(sv.v[r], ev.v[t], acc[r][t]);
       }
 #pragma unroll
       for (int r = 0; r < 4; ++r) {
         const int m = 2 * (4 * q + r) + 1 + par;
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-          const int i = 1 + c0 + 2 * cp + t;
+        for (int t = 0; t < 4; ++t) {
+          const int i = 1 + c0 + 4 * cq + t;
           if (m <= nzi && i <= nri) G[m * nr + i] = acc[r][t];
         }
       }
