@@ -23,6 +23,9 @@ using namespace ptefit;
 
 static thread_local std::string g_error;
 
+struct GraphKey { int batch, n_iter, warm; const void *p[13]; };
+struct CachedGraph { GraphKey key; cudaGraphExec_t exec; int launches; };
+
 struct ptefit_handle {
   ptefit_precision prec;
   ptefit_gemm_mode gemm;
@@ -40,6 +43,9 @@ struct ptefit_handle {
   int std_np = 0;                       // > 0: standard term list, basis generated inside the response GEMM
   CUtensorMap mapJbHi, mapJbLo, mapGpHi, mapGpLo, mapCurHi, mapCurLo, mapGbHi, mapGbLo;
   long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
+  bool use_graph = true;                // replay the launch sequence as a CUDA graph (PTEFIT_NO_GRAPH=1 disables)
+  std::vector<CachedGraph> graphs;
+  cudaStream_t gstream = nullptr;       // capture stream
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
   int fused_grid = 0;                   // resident CTAs of k_solve_fused
   size_t fused_smem = 0;
@@ -293,6 +299,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   }
   h = new ptefit_handle();
   h->prec = op->precision; h->gemm = op->gemm; h->max_batch = op->max_batch;
+  h->use_graph = getenv("PTEFIT_NO_GRAPH") == nullptr;
   ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
                                               : build(h, h->d64, g, ge, tb, ba, op->max_batch);
   if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) st = build_tc(h, h->d32, ge, tb, op->max_batch);
@@ -307,6 +314,8 @@ extern "C" void ptefit_destroy(ptefit_handle *h) {
   for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   void *hp[] = {h->hb, h->hic, h->hpsi, h->hco, h->hax, h->hxp, h->hpb, h->hchi, h->haxij, h->hxpij, h->hlim, h->hst};
   for (void *p : hp) if (p) cudaFree(p);
+  for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
+  if (h->gstream) cudaStreamDestroy(h->gstream);
   if (h->phase_clk) cudaFree(h->phase_clk);
   if (h->hstream) cudaStreamDestroy(h->hstream);
   delete h;
