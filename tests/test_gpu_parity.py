@@ -230,3 +230,44 @@ def test_paper_form_without_additions():
         else:
             assert int(out["status"][q]) == ores["status"]
     rec.close()
+
+
+@pytest.mark.parametrize("variant", ["ffma", "nonstandard_terms", "no_graph_profiling"])
+def test_fp32_code_path_variants(variant):
+    """The FP32 path has three contraction routes: tcgen05 GEMM with in-kernel basis producer (the
+    default, covered above), tcgen05 GEMM fed by k_basis_split (term lists that are not NP = NFF in
+    {2, 3}), and the plain FMA kernels (PTEFIT_GEMM_FFMA).  Each must meet the same tolerances; the
+    stage-event (non-graph) launch path must give bit-identical results to the graph replay."""
+    torch = _torch()
+    import paper_2601_12378_b200 as P
+    from paper_2601_12378_b200.binding import GEMM_FFMA
+    dev, sl = cached_case("cfg2", 2)
+    if variant == "nonstandard_terms":
+        dev = dict(dev); dev["basis"] = dict(dev["basis"], n_p=3, n_ff=2)
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    od = oracle_device(dv)
+    n_iter = 8
+    kw = dict(gemm=GEMM_FFMA) if variant == "ffma" else {}
+    rec = _rec(dev, "fp32", 2, **kw)
+    db = torch.tensor(b, dtype=rec.dtype, device="cuda"); dic = torch.tensor(ic, dtype=rec.dtype, device="cuda")
+    rec.reconstruct(db, dic, n_iter)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, 2)
+    for q in range(2):
+        ores = reconstruct(od, b[q], ic[q], n_iter)
+        assert ores["status"] == 0
+        check_slice(out, q, ores, dev, "fp32", strict_index=False)
+    if variant == "no_graph_profiling":
+        rec.reconstruct(db, dic, n_iter)                  # second call with the same arguments: graph replay
+        torch.cuda.synchronize()
+        out_replay = _gpu_out(rec, 2)
+        rec.set_profiling(True)                           # direct launches with stage events
+        rec.reconstruct(db, dic, n_iter)
+        torch.cuda.synchronize()
+        ms = rec.stage_ms()
+        rec.set_profiling(False)
+        out_direct = _gpu_out(rec, 2)
+        assert sum(ms.values()) > 0
+        for k in ("psi", "coeffs", "axis_ij", "xpt_ij", "chi2", "status"):
+            assert np.array_equal(out[k], out_replay[k]) and np.array_equal(out[k], out_direct[k]), k
+    rec.close()
