@@ -132,6 +132,7 @@ struct AProd {
   const int *cnode;           // [Kc] compact node list
   const float *rdA, *fdA;     // [Kc] R dA and mu0 dA / R of the compact nodes
   int N, B, has_delz;
+  long long *dbg;
 };
 template <int NP> constexpr int gemm_threads() { return NP > 0 ? 448 : GEMM_THREADS; }
 
@@ -196,16 +197,17 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
     if (lane == 0) {                                   // ---- MMA issuer
       constexpr uint32_t idesc = idesc_tf32(BM, BN);
       int it = 0;
+      long long w_full = 0, w_temp = 0; const long long t_start = clock64();
       for (int c = 0; c < nchunks; ++c) {
         const int buf = c & 1;
-        mbar_wait(tempty + buf, ((uint32_t)(c >> 1) & 1u) ^ 1u);       // accumulator drained by the register adders
+        { const long long t0 = clock64(); mbar_wait(tempty + buf, ((uint32_t)(c >> 1) & 1u) ^ 1u); w_temp += clock64() - t0; }
         tc_fence_after();
         const uint32_t tacc = tmem_base + (uint32_t)(buf * ACC_COLS);
         const int kend = min(kb0 + (c + 1) * DRAIN, kb1);
         for (int kb = kb0 + c * DRAIN; kb < kend; ++kb, ++it) {
           const int s = it % STAGES;
           const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
-          mbar_wait(full + s, ph);
+          { const long long t0 = clock64(); mbar_wait(full + s, ph); w_full += clock64() - t0; }
           tc_fence_after();
           const uint32_t sa = smem_u32(base + s * L::STAGE_BYTES);
           const uint64_t dAhi = smem_desc_sw128(sa), dAlo = smem_desc_sw128(sa + L::A_BYTES);
@@ -222,64 +224,89 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         }
         tc_commit(tfull + buf);                        // chunk complete
       }
+      if (ap.dbg && blockIdx.x == 0 && blockIdx.z == 0) { ap.dbg[0] += w_full; ap.dbg[1] += w_temp; ap.dbg[2] += clock64() - t_start; ap.dbg[3] += kb1 - kb0; }
     }
   } else if (NP > 0 && warp >= 10) {                   // ---- basis producers (warps 10-13)
     constexpr int NPOLY = NP + NFF;
     constexpr int PMAX = NP > NFF ? NP : NFF;
-    const int pw_ = warp - 10;                          // handles slices 4 pw_ .. 4 pw_ + 3 of the tile
-    const int sbase = m0 / 8 + 4 * pw_;
-    float xv[4], dv[4], rd, fd;
-    auto fetch = [&](int kb, float *x, float *d, float &r, float &f) {
-      const int kc = kb * BK + lane;
-      const int n = ap.cnode[kc];
-      r = ap.rdA[kc]; f = ap.fdA[kc];
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int sl = min(sbase + q, ap.B - 1);
-        x[q] = ap.xn[(size_t)sl * ap.N + n];
-        d[q] = ap.has_delz ? ap.dzc[(size_t)sl * ap.N + n] : 0.f;
-      }
+    // lane -> (slice sq = lane >> 3 of the warp's four, node quad kq = lane & 7 of the block's
+    // 32 nodes): four consecutive nodes of one slice per thread, so that every term row is one
+    // 16-byte store per hi / lo tile (a quarter warp covers one 128-byte row: conflict free).
+    const int pw_ = warp - 10, sq = lane >> 3, kq = lane & 7;
+    const int sl = min(m0 / 8 + 4 * pw_ + sq, ap.B - 1);
+    const float *xs = ap.xn + (size_t)sl * ap.N, *ds = ap.dzc + (size_t)sl * ap.N;
+    // software pipeline of the gather: node indices and factors of block kb + 3, flux values of
+    // block kb + 2 (their addresses need the indices), arithmetic of block kb
+    int4 nidx = make_int4(0, 0, 0, 0);
+    float4 nr_ = make_float4(0.f, 0.f, 0.f, 0.f), nf_ = nr_;
+    auto fetch_idx = [&](int kb) {
+      if (kb >= kb1) return;
+      const int kc = kb * BK + 4 * kq;
+      nidx = *reinterpret_cast<const int4 *>(ap.cnode + kc);
+      nr_ = *reinterpret_cast<const float4 *>(ap.rdA + kc);
+      nf_ = *reinterpret_cast<const float4 *>(ap.fdA + kc);
     };
-    if (kb0 < kb1) fetch(kb0, xv, dv, rd, fd);
-    for (int kb = kb0, it = 0; kb < kb1; ++kb, ++it) {
+    auto fetch_val = [&](int kb, float *x, float *d, float4 &r, float4 &f) {   // uses nidx = indices of block kb
+      if (kb >= kb1) return;
+      const int4 n = nidx;
+      r = nr_; f = nf_;
+      x[0] = xs[n.x]; x[1] = xs[n.y]; x[2] = xs[n.z]; x[3] = xs[n.w];
+      if (ap.has_delz) { d[0] = ds[n.x]; d[1] = ds[n.y]; d[2] = ds[n.z]; d[3] = ds[n.w]; }
+      else d[0] = d[1] = d[2] = d[3] = 0.f;
+    };
+    // one K block: consume a register buffer filled two blocks ago, refill it for block kb + 2
+    // (gather latency ~ two block times), then write the tiles of block kb
+    auto step = [&](int kb, int it, float *xb, float *db, float4 &rb, float4 &fb) {
       const int s = it % STAGES;
       const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
-      float x[4], d[4];
-      const float r = rd, f = fd;
+      float d[4];
+      const float r[4] = {rb.x, rb.y, rb.z, rb.w}, f[4] = {fb.x, fb.y, fb.z, fb.w};
+      float pwv[4][PMAX + 1];
+      bool in[4];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) { x[q] = xv[q]; d[q] = dv[q]; }
-      if (kb + 1 < kb1) fetch(kb + 1, xv, dv, rd, fd);   // next block's loads fly during this block's math
+      for (int t = 0; t < 4; ++t) {
+        d[t] = db[t];
+        pwv[t][0] = 1.f;
+#pragma unroll
+        for (int k = 1; k <= PMAX; ++k) pwv[t][k] = pwv[t][k - 1] * xb[t];
+        in[t] = !(xb[t] < 0.f);
+      }
+      fetch_val(kb + 2, xb, db, rb, fb);
+      fetch_idx(kb + 3);
       mbar_wait(empty + s, ph ^ 1u);
       unsigned char *ahi = base + s * L::STAGE_BYTES, *alo = ahi + L::A_BYTES;
+      const uint32_t rowbase = (uint32_t)(4 * pw_ + sq) * 1024u;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        float pwv[PMAX + 1];
-        pwv[0] = 1.f;
+      for (int l = 0; l < NPOLY + 1; ++l) {
+        if (l == NPOLY && !ap.has_delz) break;
+        uint32_t hr[4], lr[4];
 #pragma unroll
-        for (int k = 1; k <= PMAX; ++k) pwv[k] = pwv[k - 1] * x[q];
-        const bool in = !(x[q] < 0.f);
-        const uint32_t rowbase = (uint32_t)(4 * pw_ + q) * 1024u + (uint32_t)(lane & 3) * 4u;
-#pragma unroll
-        for (int l = 0; l < NPOLY + 1; ++l) {
+        for (int t = 0; t < 4; ++t) {
           float v;
-          if (l < NP) v = in ? (pwv[l] - pwv[NP]) * r : 0.f;
-          else if (l < NPOLY) v = in ? (pwv[l - NP] - pwv[NFF]) * f : 0.f;
-          else v = d[q];
-          if (l == NPOLY && !ap.has_delz) break;
-          const float hi = __uint_as_float(__float_as_uint(v));
-          uint32_t hr;
-          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(hr) : "f"(hi));
-          const float hf = __uint_as_float(hr);
-          uint32_t lr;
-          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(lr) : "f"(v - hf));
-          const uint32_t off = rowbase + (uint32_t)l * 128u + ((((uint32_t)lane >> 2) ^ (uint32_t)l) << 4);
-          *reinterpret_cast<uint32_t *>(ahi + off) = hr;
-          *reinterpret_cast<uint32_t *>(alo + off) = lr;
+          if (l < NP) v = in[t] ? (pwv[t][l] - pwv[t][NP]) * r[t] : 0.f;
+          else if (l < NPOLY) v = in[t] ? (pwv[t][l - NP] - pwv[t][NFF]) * f[t] : 0.f;
+          else v = d[t];
+          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(hr[t]) : "f"(v));
+          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(lr[t]) : "f"(v - __uint_as_float(hr[t])));
         }
+        const uint32_t off = rowbase + (uint32_t)l * 128u + (((uint32_t)kq ^ (uint32_t)l) << 4);
+        *reinterpret_cast<uint4 *>(ahi + off) = make_uint4(hr[0], hr[1], hr[2], hr[3]);
+        *reinterpret_cast<uint4 *>(alo + off) = make_uint4(lr[0], lr[1], lr[2], lr[3]);
       }
       fence_proxy_async();                              // generic-proxy writes -> visible to tcgen05.mma
       __syncwarp();
       if (lane == 0) mbar_arrive(full + s);
+    };
+    float xa[4], da[4], xb2[4], db2[4];
+    float4 ra, fa, rb2, fb2;
+    fetch_idx(kb0);
+    fetch_val(kb0, xa, da, ra, fa);
+    fetch_idx(kb0 + 1);
+    fetch_val(kb0 + 1, xb2, db2, rb2, fb2);
+    fetch_idx(kb0 + 2);
+    for (int kb = kb0, it = 0; kb < kb1; kb += 2, it += 2) {
+      step(kb, it, xa, da, ra, fa);
+      if (kb + 1 < kb1) step(kb + 1, it + 1, xb2, db2, rb2, fb2);
     }
   } else if (warp >= 2 && warp < 10) {                 // ---- promotion to registers + epilogue
     const int q = warp & 3;                            // TMEM lane quarter this warp may access
