@@ -271,7 +271,7 @@ def run_ours(args):
     roof = stage_roofline(top, loop_stages[top] / n_iter, dims, peaks, args.gemm)
     roof["frac"] = roof["achieved"] / roof["peak"]
     # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the committed
-    # `ncu --set full` capture of this workload, profiles/r1_v9_ncu_full.md; null for other workloads
+    # `ncu --set full` capture of this workload, profiles/r1_final_ncu_full.md; null for other workloads
     ncu_traffic = {"k_solve_fused": 216.7e6, "response": 54.1e6, "boundary": 65.8e6}
     roof["traffic"] = None
     if args.config == "cfg4" and B == 512:
