@@ -38,16 +38,16 @@ __device__ __forceinline__ Vec2<double> load2(const double *p) {
 
 // Shared-memory bytes of k_solve_fused for a grid (host and device agree through this).
 template <typename T>
-__host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
+__host__ __device__ inline size_t fused_smem_bytes(int nr, int nz, bool pre = false) {
   const int n2 = (nz - 1) / 2;
   const size_t g = ((size_t)nz * nr + 3) & ~(size_t)3;          // 16-byte aligned sub-arrays
-  size_t e = 2 * (size_t)n2 * FUSED_CW * sizeof(T);               // fold buffer, reused for the bit masks
+  size_t e = pre ? 0 : 2 * (size_t)n2 * FUSED_CW * sizeof(T);     // fold buffer, reused for the bit masks
   const size_t mb = 2 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);
   if (mb > e) e = mb;
   const size_t pbb = (size_t)(2 * (nr + nz) - 4) * sizeof(T);   // ... and for the boundary flux
   if (pbb > e) e = pbb;
   e = (e + 15) & ~(size_t)15;
-  return (g + 2 * (size_t)n2 * n2) * sizeof(T) + e;
+  return (g + (pre ? 0 : 2 * (size_t)n2 * n2)) * sizeof(T) + e;
 }
 
 // In-place DST-I along Z of the interior columns of G[nz][nr] (rows 1..nz-2 <-> modes 1..nz-2),
@@ -121,21 +121,24 @@ __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefe
 // grid min(B, resident CTAs), block FUSED_THREADS, dyn smem fused_smem_bytes<T>(nr, nz).
 // cur[B][N] node currents (A), pbd[B][nbnd] boundary flux, psi[B][N] in/out.
 // do_search = 0: Delta* solve only (debug hook); 1: also search + xn (+ dzc when has_delz).
-template <typename T>
+// pl_all != nullptr: the plasma flux of the interior nodes was already solved (split_solve.cuh):
+// load it instead of the currents and skip the solve phases.
+template <typename T, bool PRE = false>
 __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int B, const T *__restrict__ cur_all,
                                                                 const T *__restrict__ pbd_all, T *__restrict__ psi_all,
                                                                 T *__restrict__ xn_all, int use_relax, int add_coil,
-                                                                int do_search) {
+                                                                int do_search, const T *__restrict__ pl_all) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int nr = D.nr, nz = D.nz, N = D.N, nri = D.nri, nzi = D.nzi, Nz = nz - 1, n2 = Nz / 2;
   const int tid = threadIdx.x, nth = blockDim.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
   T *G = reinterpret_cast<T *>(smem_raw);
   T *So = G + ((N + 3) & ~3);
   T *Se = So + n2 * n2;
-  T *E = Se + n2 * n2;
+  T *E = PRE ? So : Se + n2 * n2;                          // PRE: no DST tables in shared memory
   unsigned *mbits = reinterpret_cast<unsigned *>(E);        // during the search: lim bits, then xpt bits
   const int nwords = (N + 31) >> 5;
-  for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];      // So then Se, contiguous
+  if (!PRE)
+    for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];    // So then Se, contiguous
   // per-column constants (same expressions as the unfused kernels, evaluated once per CTA)
   __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
   __shared__ T pcoef[2 * (PTEFIT_MAX_DEG + 1)];              // I'(x) = rdA P(x) + fdA Q(x)
@@ -151,6 +154,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
   }
   const T cz = T(1.0 / (D.dz * D.dz));
   const T scale = T(2.0 / Nz);
+  const T esc = pl_all ? T(1) : scale;             // the split path stores the flux already scaled
   const T om = T(D.relax);
   const double sg = (double)D.ip_sign;
   long long t_phase = clock64();
@@ -164,7 +168,8 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     // ---- node currents straight into shared memory (asynchronous copies, no register staging)
     for (int k = tid; k < D.nbnd; k += nth) E[k] = pbg[k];
     for (int n = tid; n < N; n += nth) {
-      if (sizeof(T) == 4) cp_async4(G + n, I + n); else cp_async8(G + n, I + n);
+      const T *src = pl_all ? pl_all + (size_t)s * N + n : I + n;
+      if (sizeof(T) == 4) cp_async4(G + n, src); else cp_async8(G + n, src);
     }
     // inputs of the later phases: pull them into L2 while the solve runs
     {
@@ -187,6 +192,17 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     cp_async_wait_all();
     __syncthreads();
     PTEFIT_PHASE(15);
+    if (PRE || pl_all) {                                   // solved elsewhere: only the edge data is missing
+      for (int k = tid; k < D.nbnd; k += nth) {
+        int n;
+        if (k < nr) n = k;
+        else if (k < 2 * nr) n = (nz - 1) * nr + (k - nr);
+        else if (k < 2 * nr + nzi) n = (k - 2 * nr + 1) * nr;
+        else n = (k - 2 * nr - nzi + 1) * nr + nr - 1;
+        G[n] = pb[k];
+      }
+      __syncthreads();
+    } else {
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
     // (one warp per grid row: the row tests are warp-uniform, the column tests plain selects)
     for (int j = warp; j < nz; j += nwarp) {
@@ -317,6 +333,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     PTEFIT_PHASE(2);
     dst_columns<T>(G, So, Se, E, nr, nz);
     PTEFIT_PHASE(3);
+    }
     // ---- bit masks of the search into the (now free) fold buffer
     if (do_search)
       for (int w = tid; w < 2 * nwords; w += nth) mbits[w] = (w < nwords) ? D.lim_bits[w] : D.xpt_bits[w - nwords];
@@ -330,9 +347,13 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
       // one warp per grid row; the global loads of a row (and of the next row) are in flight
       // before they are used
       constexpr int KR = (PTEFIT_MAX_NR + 31) / 32;
+      const T sgT = T(D.ip_sign);
+      T am_v = -INFINITY;
+      int am_n = 0x7fffffff;
       auto load_row = [&](int j, T *cv, T *ov) {
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
+          if (32 * k >= nr) break;                         // warp-uniform: rows are shorter than KR * 32
           const int i = lane + 32 * k;
           const bool ok = (j < nz) && (i < nr);
           cv[k] = (add_coil && ok) ? pc[j * nr + i] : T(0);
@@ -350,23 +371,27 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
         T *row = G + j * nr;
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
+          if (32 * k >= nr) break;
           const int i = lane + 32 * k;
           if (i < nr) {
             const bool edge = erow | (i == 0) | (i == nr - 1);
-            T v = edge ? row[i] : row[i] * scale;
+            T v = edge ? row[i] : row[i] * esc;
             v += cv[k];
             if (use_relax) v = ov[k] + om * (v - ov[k]);
             psi[j * nr + i] = v;
             row[i] = v;
             if (do_search) {
               const int n = j * nr + i;
-              const double dv = (double)v;
-              so_opt.bad |= !isfinite(dv);
-              if ((mbits[n >> 5] >> (n & 31)) & 1u) { ArgMax c; c.v = sg * dv; c.n = n; so_opt.am = better(so_opt.am, c); }
+              so_opt.bad |= !isfinite(v);
+              // arg-max key in T (exact: the keys are T values), ties -> smaller n; widened after the loop
+              const T key = sgT * v;
+              if (((mbits[n >> 5] >> (n & 31)) & 1u) && (key > am_v || (key == am_v && n < am_n))) { am_v = key; am_n = n; }
             }
           }
         }
       }
+      so_opt.am.v = (double)am_v;
+      so_opt.am.n = am_n;
     }
     __syncthreads();
     PTEFIT_PHASE(4);

@@ -18,6 +18,7 @@
 #include "fused_solve.cuh"
 #include "tc_gemm.cuh"
 #include "tc_kernels.cuh"
+#include "split_solve.cuh"
 
 using namespace ptefit;
 
@@ -40,6 +41,10 @@ struct ptefit_handle {
   const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;
   int pbd_ntiles = 0;
   const float *c_rdA = nullptr, *c_fdA = nullptr;   // Eq. 10 factors on the compact node list
+  bool split = false;                   // solve as batched DST GEMMs + tridiagonal kernel (PTEFIT_SPLIT_SOLVE)
+  SplitDev Sp{};
+  const float *s_hi = nullptr, *s_lo = nullptr;
+  CUtensorMap mapSaHi, mapSaLo, mapSxHi, mapSxLo, mapSHi, mapSLo;
   int std_np = 0;                       // > 0: standard term list, basis generated inside the response GEMM
   CUtensorMap mapJbHi, mapJbLo, mapGpHi, mapGpLo, mapCurHi, mapCurLo, mapGbHi, mapGbLo;
   long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
@@ -49,6 +54,8 @@ struct ptefit_handle {
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
   int fused_grid = 0;                   // resident CTAs of k_solve_fused
   size_t fused_smem = 0;
+  int fused_pre_grid = 0;               // lean variant of k_solve_fused used by the split solve path
+  size_t fused_pre_smem = 0;
   bool profiling = false;
   std::vector<cudaEvent_t> ev;          // stage boundaries of the last call
   std::vector<int> ev_stage;
@@ -302,7 +309,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   h->use_graph = getenv("PTEFIT_NO_GRAPH") == nullptr;
   ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
                                               : build(h, h->d64, g, ge, tb, ba, op->max_batch);
-  if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) st = build_tc(h, h->d32, ge, tb, op->max_batch);
+  if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) { st = build_tc(h, h->d32, ge, tb, op->max_batch); if (st == PTEFIT_OK) st = build_split(h, h->d32, op->max_batch); }
   if (st != PTEFIT_OK) { std::string e = h->error; ptefit_destroy(h); g_error = e; return st; }
   *out = h;
   return PTEFIT_OK;

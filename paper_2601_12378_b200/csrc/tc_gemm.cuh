@@ -132,7 +132,10 @@ struct AProd {
   const int *cnode;           // [Kc] compact node list
   const float *rdA, *fdA;     // [Kc] R dA and mu0 dA / R of the compact nodes
   int N, B, has_delz;
-  long long *dbg;
+  // epilogue of the DST products (split solve path): epi = 1 stores D[(s, i)][c] * scale transposed
+  // into the flux grid, out[s][(c + 1) nr + i + 1], rows r = s RS + i; epi = 0: plain partials
+  int epi, RS, nri, nzi, nr;
+  float scale;
 };
 template <int NP> constexpr int gemm_threads() { return NP > 0 ? 448 : GEMM_THREADS; }
 
@@ -197,17 +200,16 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
     if (lane == 0) {                                   // ---- MMA issuer
       constexpr uint32_t idesc = idesc_tf32(BM, BN);
       int it = 0;
-      long long w_full = 0, w_temp = 0; const long long t_start = clock64();
       for (int c = 0; c < nchunks; ++c) {
         const int buf = c & 1;
-        { const long long t0 = clock64(); mbar_wait(tempty + buf, ((uint32_t)(c >> 1) & 1u) ^ 1u); w_temp += clock64() - t0; }
+        mbar_wait(tempty + buf, ((uint32_t)(c >> 1) & 1u) ^ 1u);       // accumulator drained by the register adders
         tc_fence_after();
         const uint32_t tacc = tmem_base + (uint32_t)(buf * ACC_COLS);
         const int kend = min(kb0 + (c + 1) * DRAIN, kb1);
         for (int kb = kb0 + c * DRAIN; kb < kend; ++kb, ++it) {
           const int s = it % STAGES;
           const uint32_t ph = (uint32_t)(it / STAGES) & 1u;
-          { const long long t0 = clock64(); mbar_wait(full + s, ph); w_full += clock64() - t0; }
+          mbar_wait(full + s, ph);
           tc_fence_after();
           const uint32_t sa = smem_u32(base + s * L::STAGE_BYTES);
           const uint64_t dAhi = smem_desc_sw128(sa), dAlo = smem_desc_sw128(sa + L::A_BYTES);
@@ -224,7 +226,6 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         }
         tc_commit(tfull + buf);                        // chunk complete
       }
-      if (ap.dbg && blockIdx.x == 0 && blockIdx.z == 0) { ap.dbg[0] += w_full; ap.dbg[1] += w_temp; ap.dbg[2] += clock64() - t_start; ap.dbg[3] += kb1 - kb0; }
     }
   } else if (NP > 0 && warp >= 10) {                   // ---- basis producers (warps 10-13)
     constexpr int NPOLY = NP + NFF;
@@ -338,6 +339,22 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
       if (lane == 0) mbar_arrive(tempty + buf);
     }
     const int row = q * 32 + lane;
+    if (ap.epi == 1) {
+      const int r = m0 + row, sl = r / ap.RS, i = r - sl * ap.RS;
+      if (sl < ap.B && i < ap.nri) {
+        float *o = out + (size_t)sl * ap.N + i + 1;
+#pragma unroll
+        for (int g = 0; g < NCH; ++g) {
+          if (g * 16 < ncols) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+              const int c = n0 + col0 + g * 16 + k;              // mode / row index c + 1 of the grid
+              if (c < ap.nzi) o[(c + 1) * ap.nr] = acc[g][k] * ap.scale;
+            }
+          }
+        }
+      }
+    } else {
     float *o = out + ((size_t)z * gridDim.x * BM + m0 + row) * ldo + n0 + col0;
 #pragma unroll
     for (int g = 0; g < NCH; ++g) {
@@ -346,6 +363,7 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         for (int k = 0; k < 16; k += 4)
           *reinterpret_cast<float4 *>(o + g * 16 + k) = make_float4(acc[g][k], acc[g][k + 1], acc[g][k + 2], acc[g][k + 3]);
       }
+    }
     }
   }
   tc_fence_before();
