@@ -265,10 +265,13 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
         }
         ex[side * half + mm] = prev;                       // y_{k-1} (left) or y_{k+1} (right)
       }
+      // both threads of a mode need the right-hand side of row k; the left one overwrites it below,
+      // so it is read before the barrier
+      const double gk = act ? (double)row[k] : 0.0;
       __syncthreads();
       double x = 0.0;
       if (act) {
-        const double yk = (double)row[k] - __ldg(tw + (size_t)k * nzi) * ex[mm] - __ldg(D.tw2k + mm) * ex[half + mm];
+        const double yk = gk - __ldg(tw + (size_t)k * nzi) * ex[mm] - __ldg(D.tw2k + mm) * ex[half + mm];
         x = yk * __ldg(tb + (size_t)k * nzi);
         if (!side) row[k] = T(x);
         for (int t0 = len - 1; t0 >= 0; t0 -= U) {

@@ -277,3 +277,52 @@ def test_fp32_code_path_variants(variant):
         for k in ("psi", "coeffs", "axis_ij", "xpt_ij", "chi2", "status"):
             assert np.array_equal(out[k], out_replay[k]) and np.array_equal(out[k], out_direct[k]), k
     rec.close()
+
+
+def test_full_size_properties_cfg4():
+    """BASELINE config 4 at full size in the launch configuration bench.py times (129x129, batch 512,
+    20 iterations, max_batch 512): properties that hold at any size, checked on every slice.
+    (a) the Delta* solve stage satisfies the discrete 5-point equations (oracle/gs_solve.py's
+        operator applied to the GPU result), all 512 slices: a flux within 2e-6 max|psi| of the exact
+        discrete solution can leave a residual of at most |A_h|_inf 2e-6 max|psi|, |A_h|_inf = 2 (2/dR^2 + 2/dZ^2);
+    (b) after the loop: normalised quantities are consistent -- status 0 slices have the axis inside
+        the limiter mask, psi_axis > psi_bnd (I_p > 0), chi2 finite and positive;
+    (c) slices with identical inputs give bit-identical outputs wherever they sit in the batch."""
+    torch = _torch()
+    dev, sl = cached_case("cfg4", 24)
+    od = oracle_device(dev)
+    rec = _rec(dev, "fp32", 512)
+    rng = np.random.default_rng(7)
+    # (a) random smooth-ish currents inside the limiter, random boundary flux
+    N = od.nr * od.nz
+    lim = od.lim_mask.ravel()
+    I = (rng.uniform(0.0, 40.0, (512, N)) * lim[None, :]).astype(np.float32)
+    pbd = rng.uniform(-0.05, 0.05, (512, len(od.bnd))).astype(np.float32)
+    dI = torch.tensor(I, device="cuda"); dp = torch.tensor(pbd, device="cuda")
+    out = torch.zeros(512, od.nz, od.nr, dtype=torch.float32, device="cuda")
+    rec.debug_gs_solve(dI, dp, out)
+    psi = out.cpu().numpy().astype(np.float64)
+    from oracle.gs_solve import MU0
+    worst = 0.0
+    for q in range(512):
+        rhs = -MU0 * od.r[None, 1:-1] * I[q].astype(np.float64).reshape(od.nz, od.nr)[1:-1, 1:-1] / od.dA
+        res = od.op.apply(psi[q]) - rhs
+        a_inf = 2.0 * (2.0 / od.op.dr ** 2 + 2.0 / od.op.dz ** 2)
+        worst = max(worst, float(np.max(np.abs(res)) / (a_inf * 2e-6 * np.max(np.abs(psi[q])))))
+        assert np.array_equal(psi[q].ravel()[od.bnd], pbd[q].astype(np.float64))
+    assert worst <= 1.0, worst
+    # (b), (c) full reconstruction, the 24 distinct slices tiled over the batch
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    bb = np.tile(b, (22, 1))[:512]; icc = np.tile(ic, (22, 1))[:512]
+    rec.reconstruct(torch.tensor(bb, dtype=rec.dtype, device="cuda"), torch.tensor(icc, dtype=rec.dtype, device="cuda"), 20)
+    torch.cuda.synchronize()
+    o = _gpu_out(rec, 512)
+    ok = o["status"] == 0
+    assert ok.sum() >= 500
+    ai, aj = o["axis_ij"][ok, 0], o["axis_ij"][ok, 1]
+    assert np.all(od.lim_mask[aj, ai])
+    assert np.all(o["axis_rzpsi"][ok, 2] > o["psi_bnd"][ok])
+    assert np.all(np.isfinite(o["chi2"][ok])) and np.all(o["chi2"][ok] > 0)
+    for q in range(24, 512):
+        assert np.array_equal(o["psi"][q], o["psi"][q % 24]) and np.array_equal(o["coeffs"][q], o["coeffs"][q % 24])
+    rec.close()
