@@ -287,7 +287,9 @@ def test_full_size_properties_cfg4():
         discrete solution can leave a residual of at most |A_h|_inf 2e-6 max|psi|, |A_h|_inf = 2 (2/dR^2 + 2/dZ^2);
     (b) after the loop: normalised quantities are consistent -- status 0 slices have the axis inside
         the limiter mask, psi_axis > psi_bnd (I_p > 0), chi2 finite and positive;
-    (c) slices with identical inputs give bit-identical outputs wherever they sit in the batch."""
+    (c) slices with identical inputs give bit-identical outputs wherever they sit in the batch;
+    (d) axis index = numpy arg-max of the returned flux over the limiter mask, all slices;
+    (e) repeated calls give bit-identical outputs."""
     torch = _torch()
     dev, sl = cached_case("cfg4", 24)
     od = oracle_device(dev)
@@ -325,4 +327,16 @@ def test_full_size_properties_cfg4():
     assert np.all(np.isfinite(o["chi2"][ok])) and np.all(o["chi2"][ok] > 0)
     for q in range(24, 512):
         assert np.array_equal(o["psi"][q], o["psi"][q % 24]) and np.array_equal(o["coeffs"][q], o["coeffs"][q % 24])
+    # (d) the axis node of every slice is the arg-max of psi over the limiter mask (tie -> smallest index),
+    #     recomputed here from the returned flux with numpy: bit-exact on all 512 slices
+    sp = np.where(od.lim_mask.ravel()[None, :], o["psi"].reshape(512, -1).astype(np.float64), -np.inf)
+    na = np.argmax(sp, axis=1)
+    assert np.array_equal(o["axis_ij"][ok, 0], (na % od.nr)[ok]) and np.array_equal(o["axis_ij"][ok, 1], (na // od.nr)[ok])
+    # (e) run-to-run reproducibility of every output (a data race shows up here)
+    for _ in range(2):
+        rec.reconstruct(torch.tensor(bb, dtype=rec.dtype, device="cuda"), torch.tensor(icc, dtype=rec.dtype, device="cuda"), 20)
+        torch.cuda.synchronize()
+        o2 = _gpu_out(rec, 512)
+        for k in o:
+            assert np.array_equal(o[k], o2[k], equal_nan=True) if o[k].dtype.kind == "f" else np.array_equal(o[k], o2[k]), k
     rec.close()
