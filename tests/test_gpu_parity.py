@@ -340,3 +340,36 @@ def test_full_size_properties_cfg4():
         for k in o:
             assert np.array_equal(o[k], o2[k], equal_nan=True) if o[k].dtype.kind == "f" else np.array_equal(o[k], o2[k]), k
     rec.close()
+
+
+@pytest.mark.parametrize("name,precision,B", [("cfg1", "fp64", 300), ("cfg2", "fp32", 300), ("cfg2", "fp64", 96),
+                                               ("cfg3", "fp64", 40), ("cfg5", "fp32", 8), ("cfg5", "fp64", 8)])
+def test_solve_residual_many_slices(name, precision, B):
+    """Discrete-residual property of the Delta* solve stage on many slices at once, for every solve
+    route: fused kernel FP32 / FP64 (33, 65, 129 grids), three-kernel path (257 grid).  A flux
+    within `rel` max|psi| of the exact discrete solution leaves a residual <= |A_h|_inf rel max|psi|."""
+    torch = _torch()
+    import synth
+    dev = synth.make_device(name)
+    synth.make_slices(dev, 1)                        # fills sigma
+    od = oracle_device(dev)
+    rec = _rec(dev, precision, B)
+    rng = np.random.default_rng(11)
+    N = od.nr * od.nz
+    npdt = np.float32 if precision == "fp32" else np.float64
+    I = (rng.uniform(0.0, 40.0, (B, N)) * od.lim_mask.ravel()[None, :]).astype(npdt)
+    pbd = rng.uniform(-0.05, 0.05, (B, len(od.bnd))).astype(npdt)
+    out = torch.zeros(B, od.nz, od.nr, dtype=rec.dtype, device="cuda")
+    rec.debug_gs_solve(torch.tensor(I, device="cuda"), torch.tensor(pbd, device="cuda"), out)
+    psi = out.cpu().numpy().astype(np.float64)
+    from oracle.gs_solve import MU0
+    rel = 2e-6 if precision == "fp32" else 2e-13
+    a_inf = 2.0 * (2.0 / od.op.dr ** 2 + 2.0 / od.op.dz ** 2)
+    worst = 0.0
+    for q in range(B):
+        rhs = -MU0 * od.r[None, 1:-1] * I[q].astype(np.float64).reshape(od.nz, od.nr)[1:-1, 1:-1] / od.dA
+        res = od.op.apply(psi[q]) - rhs
+        worst = max(worst, float(np.max(np.abs(res)) / (a_inf * rel * np.max(np.abs(psi[q])))))
+        assert np.array_equal(psi[q].ravel()[od.bnd], pbd[q].astype(np.float64))
+    assert worst <= 1.0, worst
+    rec.close()
