@@ -289,7 +289,8 @@ def test_full_size_properties_cfg4():
         the limiter mask, psi_axis > psi_bnd (I_p > 0), chi2 finite and positive;
     (c) slices with identical inputs give bit-identical outputs wherever they sit in the batch;
     (d) axis index = numpy arg-max of the returned flux over the limiter mask, all slices;
-    (e) repeated calls give bit-identical outputs."""
+    (e) repeated calls give bit-identical outputs;
+    (f) the search of a 64-slice sample, run at full occupancy, equals the oracle's search bit for bit."""
     torch = _torch()
     dev, sl = cached_case("cfg4", 24)
     od = oracle_device(dev)
@@ -332,6 +333,27 @@ def test_full_size_properties_cfg4():
     sp = np.where(od.lim_mask.ravel()[None, :], o["psi"].reshape(512, -1).astype(np.float64), -np.inf)
     na = np.argmax(sp, axis=1)
     assert np.array_equal(o["axis_ij"][ok, 0], (na % od.nr)[ok]) and np.array_equal(o["axis_ij"][ok, 1], (na // od.nr)[ok])
+    # (f) the search stage under full occupancy: all 512 final flux maps through ptefit_debug_search, a sample
+    #     of 64 slices (both scheduling rounds of the persistent kernel) against the oracle's search: bit-exact
+    psi_t = rec.psi.clone()
+    xn = torch.zeros(512, od.nz * od.nr, dtype=rec.dtype, device="cuda")
+    rec.debug_search(psi_t, xn)
+    torch.cuda.synchronize()
+    xh = xn.cpu().numpy().astype(np.float64).reshape(512, od.nz, od.nr)
+    for q in range(3, 512, 8):
+        if int(rec.status[q]) != 0:
+            continue
+        sr = OS.search(o["psi"][q].astype(np.float64), od.r, od.z, od.lim_mask, od.xpt_mask, od.lim_r, od.lim_z, od.s)
+        assert sr["status"] == 0
+        assert tuple(rec.axis_ij[q].tolist()) == (sr["axis"][0], sr["axis"][1])
+        assert tuple(rec.xpt_ij[q].tolist()) == (sr["xpt"][0], sr["xpt"][1])
+        assert int(rec.limited[q]) == sr["limited"]
+        assert np.array_equal(xh[q] >= 0, sr["mask"])
+        assert np.max(np.abs(xh[q][sr["mask"]] - sr["psin"][sr["mask"]])) <= 2e-7
+        # ... and so do the outputs of the reconstruct call itself (search fused behind the solve)
+        assert tuple(o["axis_ij"][q]) == (sr["axis"][0], sr["axis"][1]) and tuple(o["xpt_ij"][q]) == (sr["xpt"][0], sr["xpt"][1])
+        assert int(o["limited"][q]) == sr["limited"]
+        assert abs(float(o["psi_bnd"][q]) - sr["psi_b"]) <= 1e-6 * abs(sr["psi_b"])
     # (e) run-to-run reproducibility of every output (a data race shows up here)
     for _ in range(2):
         rec.reconstruct(torch.tensor(bb, dtype=rec.dtype, device="cuda"), torch.tensor(icc, dtype=rec.dtype, device="cuda"), 20)
