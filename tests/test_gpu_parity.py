@@ -395,3 +395,34 @@ def test_solve_residual_many_slices(name, precision, B):
         assert np.array_equal(psi[q].ravel()[od.bnd], pbd[q].astype(np.float64))
     assert worst <= 1.0, worst
     rec.close()
+
+
+def test_response_fit_full_batch_cfg4():
+    """The response contraction and the fit at the full batch of config 4 (32 row tiles x 4 K splits of the
+    tcgen05 GEMM): 24 oracle states tiled over 512 slices; every slice against the oracle's response matrix
+    (numpy matmul) and coefficients, replicas bit-identical across tiles."""
+    torch = _torch()
+    from tests.helpers import coef_rel_err
+    dev, sl = cached_case("cfg4", 24)
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    od = oracle_device(dv)
+    ores = [reconstruct(od, b[q], ic[q], 3, trace=True) for q in range(24)]
+    hk = [o["hist"][2] for o in ores]; prev = [o["hist"][1] for o in ores]
+    rec = _rec(dev, "fp32", 512)
+    dt = rec.dtype
+    til = lambda a: np.tile(a, (22,) + (1,) * (a.ndim - 1))[:512]
+    xin = np.stack([np.where(p["srch"]["mask"], p["srch"]["psin"], -1.0).ravel() for p in prev])
+    resp = torch.zeros(512, od.gp.shape[0], rec.nt, dtype=dt, device="cuda")
+    rec.debug_fit(torch.tensor(til(xin), dtype=dt, device="cuda"), torch.tensor(til(b), dtype=dt, device="cuda"),
+                  torch.tensor(til(ic), dtype=dt, device="cuda"), torch.tensor(til(np.stack([p["X"] for p in prev])), dtype=dt, device="cuda"), resp)
+    torch.cuda.synchronize()
+    r = resp.cpu().numpy().astype(np.float64)
+    X = rec.coeffs.cpu().numpy().astype(np.float64)
+    for q in range(512):
+        r_or = hk[q % 24]["resp"]
+        cs = np.max(np.abs(r_or), axis=0)
+        assert np.max(np.abs(r[q] - r_or) / cs) <= 5e-6, q
+        assert coef_rel_err(X[q], hk[q % 24]["X"], od.n_p, od.n_ff, od.op.dz) <= 1e-4, q
+        if q >= 24:
+            assert np.array_equal(r[q], r[q % 24]) and np.array_equal(X[q], X[q % 24])
+    rec.close()
