@@ -39,6 +39,7 @@ struct Dev {
   const double *inv_sigma;        // [M]
   const uint8_t *lim_mask, *xpt_mask;
   const unsigned *lim_bits, *xpt_bits;   // the same masks bit-packed: bit (n & 31) of word n >> 5
+  const unsigned *edge_bits;             // bit set for the nodes of the grid edge
   const double *lim_r, *lim_z;    // [nlim]
   // Delta* solve factors: [nri][nzi] (i-major so that threads over m coalesce)
   const double *tri_w, *tri_invb; // Thomas multipliers and inverse pivots

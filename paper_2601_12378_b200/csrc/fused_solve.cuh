@@ -42,7 +42,7 @@ __host__ __device__ inline size_t fused_smem_bytes(int nr, int nz, bool pre = fa
   const int n2 = (nz - 1) / 2;
   const size_t g = ((size_t)nz * nr + 3) & ~(size_t)3;          // 16-byte aligned sub-arrays
   size_t e = pre ? 0 : 2 * (size_t)n2 * FUSED_CW * sizeof(T);     // fold buffer, reused for the bit masks
-  const size_t mb = 2 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);
+  const size_t mb = 3 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);   // lim, xpt, edge bit masks
   if (mb > e) e = mb;
   const size_t pbb = (size_t)(2 * (nr + nz) - 4) * sizeof(T);   // ... and for the boundary flux
   if (pbb > e) e = pbb;
@@ -338,8 +338,8 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     PTEFIT_PHASE(3);
     }
     // ---- bit masks of the search into the (now free) fold buffer
-    if (do_search)
-      for (int w = tid; w < 2 * nwords; w += nth) mbits[w] = (w < nwords) ? D.lim_bits[w] : D.xpt_bits[w - nwords];
+    for (int w = tid; w < 3 * nwords; w += nth)
+      mbits[w] = (w < nwords) ? D.lim_bits[w] : (w < 2 * nwords) ? D.xpt_bits[w - nwords] : D.edge_bits[w - 2 * nwords];
     __syncthreads();
     // ---- total flux + relaxation; psi goes to global memory and stays in G for the search.
     // Global loads are issued in batches of EB before use; pass 0 of the search (finiteness and
@@ -347,48 +347,36 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     SearchOpt<T> so_opt;
     so_opt.am.v = -INFINITY; so_opt.am.n = 0x7fffffff;
     {
-      // one warp per grid row; the global loads of a row (and of the next row) are in flight
-      // before they are used
-      constexpr int KR = (PTEFIT_MAX_NR + 31) / 32;
+      // flat over the nodes (coalesced, no index arithmetic: edge nodes from a bit mask); the global
+      // loads of a batch are issued before use; the arg-max key is kept in T (exact) and widened below
+      constexpr int EB = 8;
+      const unsigned *ebits = mbits + 2 * nwords;
       const T sgT = T(D.ip_sign);
       T am_v = -INFINITY;
       int am_n = 0x7fffffff;
-      auto load_row = [&](int j, T *cv, T *ov) {
+      for (int n0 = tid; n0 < N; n0 += EB * nth) {
+        T cv[EB], ov[EB];
 #pragma unroll
-        for (int k = 0; k < KR; ++k) {
-          if (32 * k >= nr) break;                         // warp-uniform: rows are shorter than KR * 32
-          const int i = lane + 32 * k;
-          const bool ok = (j < nz) && (i < nr);
-          cv[k] = (add_coil && ok) ? pc[j * nr + i] : T(0);
-          ov[k] = (use_relax && ok) ? psi[j * nr + i] : T(0);
+        for (int u = 0; u < EB; ++u) {
+          const int n = n0 + u * nth;
+          cv[u] = (add_coil && n < N) ? pc[n] : T(0);
+          ov[u] = (use_relax && n < N) ? psi[n] : T(0);
         }
-      };
-      T cn[KR], on[KR];
-      load_row(warp, cn, on);
-      for (int j = warp; j < nz; j += nwarp) {
-        T cv[KR], ov[KR];
 #pragma unroll
-        for (int k = 0; k < KR; ++k) { cv[k] = cn[k]; ov[k] = on[k]; }
-        load_row(j + nwarp, cn, on);
-        const bool erow = (j == 0) | (j == nz - 1);
-        T *row = G + j * nr;
-#pragma unroll
-        for (int k = 0; k < KR; ++k) {
-          if (32 * k >= nr) break;
-          const int i = lane + 32 * k;
-          if (i < nr) {
-            const bool edge = erow | (i == 0) | (i == nr - 1);
-            T v = edge ? row[i] : row[i] * esc;
-            v += cv[k];
-            if (use_relax) v = ov[k] + om * (v - ov[k]);
-            psi[j * nr + i] = v;
-            row[i] = v;
+        for (int u = 0; u < EB; ++u) {
+          const int n = n0 + u * nth;
+          if (n < N) {
+            const unsigned bit = 1u << (n & 31);
+            const T g = G[n];
+            T v = (ebits[n >> 5] & bit) ? g : g * esc;
+            v += cv[u];
+            if (use_relax) v = ov[u] + om * (v - ov[u]);
+            psi[n] = v;
+            G[n] = v;
             if (do_search) {
-              const int n = j * nr + i;
               so_opt.bad |= !isfinite(v);
-              // arg-max key in T (exact: the keys are T values), ties -> smaller n; widened after the loop
               const T key = sgT * v;
-              if (((mbits[n >> 5] >> (n & 31)) & 1u) && (key > am_v || (key == am_v && n < am_n))) { am_v = key; am_n = n; }
+              if ((mbits[n >> 5] & bit) && (key > am_v || (key == am_v && n < am_n))) { am_v = key; am_n = n; }
             }
           }
         }

@@ -165,6 +165,11 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
     }
     TRY(upload(h, &D.lim_bits, lb.data(), lb.size()));
     TRY(upload(h, &D.xpt_bits, xb.data(), xb.size()));
+    std::vector<unsigned> eb((N + 31) / 32, 0u);
+    for (int j = 0; j < D.nz; ++j)
+      for (int i = 0; i < D.nr; ++i)
+        if (i == 0 || j == 0 || i == D.nr - 1 || j == D.nz - 1) { const size_t n = (size_t)j * D.nr + i; eb[n >> 5] |= 1u << (n & 31); }
+    TRY(upload(h, &D.edge_bits, eb.data(), eb.size()));
   }
   TRY(upload(h, &D.lim_r, ge->lim_r, (size_t)D.nlim));
   TRY(upload(h, &D.lim_z, ge->lim_z, (size_t)D.nlim));
