@@ -398,14 +398,12 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
         __syncthreads();
         T *dzc = D.dzc + (size_t)s * N;
         const T hz = T(0.5 / D.dz);
-        for (int j = warp; j < nz; j += nwarp) {
-          const bool irow = (j >= 1) & (j <= nz - 2);
-          const T *row = G + j * nr;
-          for (int i = lane; i < nr; i += 32) {
-            T out = T(0);
-            if (irow && i >= 1 && i <= nr - 2) out = -(row[i + nr] - row[i - nr]) * hz;
-            dzc[j * nr + i] = out;
-          }
+        const unsigned *ebits = mbits + 2 * nwords;        // the masks are still in the fold buffer
+#pragma unroll 4
+        for (int n = tid; n < N; n += nth) {
+          const bool edge = (ebits[n >> 5] >> (n & 31)) & 1u;
+          const int up = edge ? n : n + nr, dn = edge ? n : n - nr;
+          dzc[n] = edge ? T(0) : -(G[up] - G[dn]) * hz;
         }
       }
       PTEFIT_PHASE(6);
