@@ -12,9 +12,16 @@ blocking, fusion or reordering beyond what the cited definition states.
 Pin status:
   greens   : pinned (quadrature of Eq. 3-5, golden values, reciprocity, B = curl psi)
   gs_solve : pinned (Solov'ev closed form, dense solve, discrete residual)
-  search   : fit/classification pinned (exact quadratics, brute force);
-             plasma-region rule = DESIGN.md reading, **parity unpinned by the paper**
-  basis    : pinned (Eq. 10 closed forms at hand-computable points)
-  lsq      : pinned (normal-equation identity, exact-data recovery)
-  picard   : pinned (fixed-point property, chi2 statistics); no printed example in the paper
+  search   : fit/classification pinned (exact quadratics, brute force); bilinear pinned (exact on
+             a linear field), cold_start pinned (hand values), limiter-vertex validity pinned by
+             constructed fluxes (behind an X-point: rejected; in front: wins);
+             the plasma-region rule itself = DESIGN.md reading, **parity unpinned by the paper**
+  basis    : pinned (Eq. 10 closed forms at hand-computable points); tension-spline cardinals
+             pinned (tau->0 = scipy natural CubicSpline, tau->inf = hat functions, partition of
+             unity, the defining ODE by finite differences, C2 at the knots) -- the spline terms
+             are BASELINE.json's, not the paper's: **parity unpinned by the paper**
+  lsq      : pinned (normal-equation identity, exact-data recovery, chi^2 follows the chi-square
+             law with M - nb degrees of freedom on forward-chain data + noise)
+  picard   : pinned (fixed-point property, exact-data recovery in one iteration, warm = continued
+             cold start); no printed example in the paper
 """

@@ -40,7 +40,9 @@ class Device:
         self.lam = basis.get("lambda_reg", 0.0)
         self.delz = int(basis.get("delz", 0))          # 1 = append the vertical-shift term
         self.relax = float(basis.get("relax", 1.0))     # psi^{k+1} = psi^k + relax (psi_new - psi^k)
-        self.nb = self.n_p + self.n_ff + self.delz
+        self.spline = basis.get("spline")               # dict(knots, tension, terms) or None (config 5: FF' edge terms)
+        self.n_spl = 0 if self.spline is None else len(self.spline["terms"])
+        self.nb = self.n_p + self.n_ff + self.n_spl + self.delz
 
 
 def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None):
@@ -48,10 +50,11 @@ def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None):
     I (node currents), psi_bdry and the search result `srch` of the new psi.
     X_prev: previous coefficients (for the delz column); psi_prev: flux to relax towards/from
     (None = take the new flux as is)."""
-    Jb = _basis.basis_columns(psin, mask, dev.r, dev.dA, dev.n_p, dev.n_ff)     # Eq. 10
+    Jb = _basis.basis_columns(psin, mask, dev.r, dev.dA, dev.n_p, dev.n_ff, dev.spline)     # Eq. 10
     Jb = Jb.reshape(-1, Jb.shape[-1]) * dev.interior[:, None]                     # edge nodes carry no current
     if dev.delz:
-        xp = np.zeros(dev.n_p + dev.n_ff) if X_prev is None else np.asarray(X_prev)[:dev.n_p + dev.n_ff]
+        nj = dev.n_p + dev.n_ff + dev.n_spl
+        xp = np.zeros(nj) if X_prev is None else np.asarray(X_prev)[:nj]
         col = _basis.delz_column(Jb, xp, dev.nz, dev.nr, dev.op.dz) * dev.interior
         Jb = np.concatenate([Jb, col[:, None]], axis=1)
     resp = dev.gp @ Jb                                                            # Eq. 6: R = G_P J_b
