@@ -31,9 +31,11 @@ typedef enum {
 
 typedef enum { PTEFIT_FP32 = 0, PTEFIT_FP64 = 1 } ptefit_precision;
 /* Arithmetic of the two dense contractions (R = G_P J_b and psi_bdry = G_B I) in FP32 mode:
- * 3xTF32 = error-compensated tensor-core products (FP32-accurate), TF32 = single pass,
- * FFMA = plain FP32 FMA.  FP64 mode always uses FP64 arithmetic. */
-typedef enum { PTEFIT_GEMM_3XTF32 = 0, PTEFIT_GEMM_TF32 = 1, PTEFIT_GEMM_FFMA = 2 } ptefit_gemm_mode;
+ * 3xTF32 = error-compensated tcgen05 tensor-core products (FP32-accurate), FFMA = plain FP32 FMA
+ * (which also selects the FMA route of the Delta* solve).  Value 1 is reserved (a single-pass TF32
+ * mode fails the parity tolerances, SURVEY.md hard part 2) and rejected by ptefit_create.
+ * FP64 mode always uses FP64 arithmetic: DMMA (mma.sync f64) tensor-core products. */
+typedef enum { PTEFIT_GEMM_3XTF32 = 0, PTEFIT_GEMM_FFMA = 2 } ptefit_gemm_mode;
 
 /* Grid.  nz-1 must be a power of two in [8, 256] (DST length); nr in [5, 257]. */
 typedef struct { int nr, nz; double rmin, rmax, zmin, zmax; } ptefit_grid;
@@ -61,22 +63,46 @@ typedef struct {
   const double *ggc;  /* [nz*nr][n_coil] flux/rad at node n per unit coil current               */
 } ptefit_tables;
 
-/* One basis term (a column of J_b, Eq. 10).  kind 0: P' term  R (x^i - x^N) dA;
- * kind 1: FF' term (mu0/R)(x^i - x^N) dA;  kind 2: vertical-shift term -dI'/dZ (DESIGN.md
- * reading O4b; i, N ignored; must be the last term, at most one).  x = normalised flux. */
-typedef struct { int kind; int i; int N; } ptefit_term;
+/* One basis term (a column of J_b, Eq. 10).  x = normalised flux.
+ * kind 0: P' term, factor R dA;  kind 1: FF' term, factor (mu0/R) dA;  kind 2: vertical-shift term
+ * -dI'/dZ (reading O4b; must be the last term, at most one; other fields ignored).
+ * family 0 (POLY_EDGE0): x^i - x^N, 0 <= i < N <= 8.
+ * family 1 (TENSION_SPLINE): cardinal tension spline phi_i(x) on `knots` (n_knots in [3,16], strictly
+ *   increasing, HOST pointer read during create) with tension `tension` > 0; zero outside
+ *   [knots[0], knots[n_knots-1]]; i = which cardinal function (BASELINE.json configs[4]; definition
+ *   in DESIGN.md reading O4c -- not in the paper).  All spline terms of a basis must share one knot
+ *   set and tension; kind must be 0 or 1. */
+typedef struct {
+  int kind, family;
+  int i, N;
+  int n_knots;
+  const double *knots;
+  double tension;
+} ptefit_term;
 
 typedef struct {
-  int n_terms;                 /* 1..12                                                         */
+  int n_terms;                 /* 1..16                                                         */
   const ptefit_term *terms;    /* HOST                                                          */
   double lambda_reg;           /* Tikhonov weight in equilibrated coordinates; 0 = Eq. 6 as is  */
   double relax;                /* psi^{k+1} = psi^k + relax (psi_new - psi^k); 1 = plain Picard */
+  int lsq_method;              /* 0 = normal equations + Cholesky, 1 = modified Gram-Schmidt QR
+                                  (the two drivers of PAPER.md:116)                             */
+  int fit_coils;               /* 1 = joint fit of the coil currents, Eq. 7:
+                                  unknowns [X; I_C'], extra rows I_C' = I_C weighted 1/sigma_ic  */
+  const double *sigma_ic;      /* [n_coil] HOST, 1-sigma of the measured coil currents (fit_coils) */
 } ptefit_basis;
+
+/* Option flags (ptefit_options.flags); 0 = defaults. */
+#define PTEFIT_OPT_NO_GRAPH 1        /* launch the kernels directly instead of replaying a CUDA graph   */
+#define PTEFIT_OPT_NO_FUSED_BASIS 2  /* materialise J_b in HBM instead of generating it in the GEMM     */
+#define PTEFIT_OPT_SOLVE_FFMA 4      /* Delta* solve with FP32-FMA DSTs instead of the tcgen05 kernel   */
 
 typedef struct {
   ptefit_precision precision;
   ptefit_gemm_mode gemm;
   int max_batch;               /* largest batch ptefit_reconstruct will be called with          */
+  int flags;                   /* PTEFIT_OPT_* bit mask                                         */
+  int tc_split_k;              /* split-K factor of the tensor-core contractions; 0 = automatic */
 } ptefit_options;
 
 /* Build a reconstruction handle: validates, copies the tables to the device (rounded to nearest
@@ -89,8 +115,12 @@ ptefit_status ptefit_create(const ptefit_grid *grid, const ptefit_geometry *geom
 
 /* Reconstruct `batch` independent time slices (1 <= batch <= max_batch), n_iter Picard
  * iterations each.  Every d_* pointer is caller-owned DEVICE memory; `real` per precision.
- * Asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream); no host
- * synchronisation, no allocation.  Outputs that are NULL are skipped (d_psi, d_coeffs required).
+ * Asynchronous on `cuda_stream` (a cudaStream_t, NULL = default stream).  The launch sequence
+ * of a (batch, n_iter, warm_start) combination is captured into a CUDA graph the first time it is
+ * seen (that call instantiates the graph: it allocates and synchronises an internal stream);
+ * every later call with the same combination only updates the graph's kernel arguments for the
+ * pointers passed and launches it: no allocation, no host synchronisation.
+ * Outputs that are NULL are skipped (d_psi, d_coeffs required).
  * Numerical failure of a slice is reported in d_status[slice] and never aborts the batch:
  * 0 ok, 1 plasma lost, 2 non-finite, 3 singular fit, 4 more than 32 X-point candidates.
  * After a failure the slice's other outputs are unspecified. */
@@ -139,13 +169,6 @@ int ptefit_last_launch_count(const ptefit_handle *h);
  * Synchronises the stream. */
 ptefit_status ptefit_set_profiling(ptefit_handle *h, int on);
 ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
-
-/* In-kernel phase timers of k_solve_fused (tuning aid): on = 1 enables them (one CTA's thread 0
- * accumulates SM-clock cycles per phase: 0 rhs, 1 DST, 2 Thomas, 3 DST, 4 total flux, 5 search,
- * 6 delz column; 8..13 sub-phases of the search: arg-max reduce, axis fit, candidates, limiter,
- * boundary flux, mask + normalisation); with out != NULL the accumulated cycles are copied to
- * out[16] (HOST) and reset.  Synchronises the device. */
-ptefit_status ptefit_debug_phase_clocks(ptefit_handle *h, int on, long long out[16]);
 
 void ptefit_destroy(ptefit_handle *h);
 const char *ptefit_last_error(const ptefit_handle *h);

@@ -11,11 +11,13 @@ LIB_PATH = os.path.join(HERE, "libptefit.so")
 EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
-    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_debug_phase_clocks",
+    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
-GEMM_3XTF32, GEMM_TF32, GEMM_FFMA = 0, 1, 2
+GEMM_3XTF32, GEMM_FFMA = 0, 2
+OPT_NO_GRAPH, OPT_NO_FUSED_BASIS, OPT_SOLVE_FFMA = 1, 2, 4
+FAMILY_POLY, FAMILY_SPLINE = 0, 1
 
 
 class PtefitError(RuntimeError):
@@ -39,15 +41,17 @@ class _Tables(C.Structure):
 
 
 class _Term(C.Structure):
-    _fields_ = [("kind", C.c_int), ("i", C.c_int), ("N", C.c_int)]
+    _fields_ = [("kind", C.c_int), ("family", C.c_int), ("i", C.c_int), ("N", C.c_int), ("n_knots", C.c_int),
+                ("knots", C.c_void_p), ("tension", C.c_double)]
 
 
 class _Basis(C.Structure):
-    _fields_ = [("n_terms", C.c_int), ("terms", C.POINTER(_Term)), ("lambda_reg", C.c_double), ("relax", C.c_double)]
+    _fields_ = [("n_terms", C.c_int), ("terms", C.POINTER(_Term)), ("lambda_reg", C.c_double), ("relax", C.c_double),
+                ("lsq_method", C.c_int), ("fit_coils", C.c_int), ("sigma_ic", C.c_void_p)]
 
 
 class _Options(C.Structure):
-    _fields_ = [("precision", C.c_int), ("gemm", C.c_int), ("max_batch", C.c_int)]
+    _fields_ = [("precision", C.c_int), ("gemm", C.c_int), ("max_batch", C.c_int), ("flags", C.c_int), ("tc_split_k", C.c_int)]
 
 
 _lib = None
@@ -86,18 +90,30 @@ def load_library():
         lib.ptefit_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.ptefit_get_stage_ms.restype = C.c_int
         lib.ptefit_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
-        lib.ptefit_debug_phase_clocks.restype = C.c_int
-        lib.ptefit_debug_phase_clocks.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong)]
         _lib = lib
     return _lib
 
 
-def poly_terms(n_p, n_ff, delz=False):
-    """Eq. 10 term list: P' terms x^i - x^n_p (i < n_p), FF' terms x^j - x^n_ff, optional delz."""
+def poly_terms(n_p, n_ff, delz=False, spline=None):
+    """Eq. 10 term list: P' terms x^i - x^n_p (i < n_p), FF' terms x^j - x^n_ff, optional FF'-type
+    tension-spline terms (spline = dict(knots, tension, terms)), optional delz.  Each term is
+    (kind, i, N) or (kind, i, N, family, knots, tension)."""
     t = [(0, i, n_p) for i in range(n_p)] + [(1, j, n_ff) for j in range(n_ff)]
+    if spline is not None:
+        kn = np.ascontiguousarray(spline["knots"], np.float64)
+        t += [(1, int(q), 0, FAMILY_SPLINE, kn, float(spline["tension"])) for q in spline["terms"]]
     if delz:
         t.append((2, 0, 0))
     return t
+
+
+def _term_struct(t, keep):
+    if len(t) == 3:
+        return _Term(int(t[0]), FAMILY_POLY, int(t[1]), int(t[2]), 0, None, 0.0)
+    kind, i, N, fam, kn, tau = t
+    kn = np.ascontiguousarray(kn, np.float64)
+    keep.append(kn)
+    return _Term(int(kind), int(fam), int(i), int(N), len(kn), _ptr(kn), float(tau))
 
 
 def _f64(a):
@@ -108,7 +124,8 @@ def _ptr(a):
     return a.ctypes.data_as(C.c_void_p) if a is not None else None
 
 
-def ptefit_create(grid, geom, tables, terms, lambda_reg, relax, precision, gemm, max_batch):
+def ptefit_create(grid, geom, tables, terms, lambda_reg, relax, precision, gemm, max_batch, flags=0, tc_split_k=0,
+                  lsq_method=0, fit_coils=0, sigma_ic=None):
     """Marshal numpy inputs into the C structs and call ptefit_create.  Returns the handle."""
     lib = load_library()
     g = _Grid(int(grid["nr"]), int(grid["nz"]), grid["rmin"], grid["rmax"], grid["zmin"], grid["zmax"])
@@ -120,9 +137,11 @@ def ptefit_create(grid, geom, tables, terms, lambda_reg, relax, precision, gemm,
                    _ptr(keep["lim_r"]), _ptr(keep["lim_z"]), _ptr(keep["lim_mask"]), _ptr(keep["xpt_mask"]),
                    int(geom.get("ip_sign", 1)), geom["cold_rc"], geom["cold_zc"], geom["cold_a"], geom["cold_b"])
     tb = _Tables(_ptr(keep["gp"]), _ptr(keep["gc"]), _ptr(keep["gb"]), _ptr(keep["ggc"]))
-    tarr = (_Term * len(terms))(*[_Term(*t) for t in terms])
-    ba = _Basis(len(terms), tarr, float(lambda_reg), float(relax))
-    op = _Options(int(precision), int(gemm), int(max_batch))
+    kk = []
+    tarr = (_Term * len(terms))(*[_term_struct(t, kk) for t in terms])
+    sic = None if sigma_ic is None else _f64(sigma_ic)
+    ba = _Basis(len(terms), tarr, float(lambda_reg), float(relax), int(lsq_method), int(fit_coils), _ptr(sic))
+    op = _Options(int(precision), int(gemm), int(max_batch), int(flags), int(tc_split_k))
     h = C.c_void_p()
     st = lib.ptefit_create(C.byref(g), C.byref(ge), C.byref(tb), C.byref(ba), C.byref(op), C.byref(h))
     if st != 0:
@@ -155,14 +174,15 @@ def ptefit_reconstruct(h, batch, d_b, d_ic, n_iter, warm_start, d_psi, d_coeffs,
 class Reconstructor:
     """Convenience owner of a handle plus output tensors (argument marshalling only)."""
 
-    def __init__(self, dev, precision="fp32", gemm=GEMM_3XTF32, max_batch=1, delz=None, lambda_reg=None, relax=None):
+    def __init__(self, dev, precision="fp32", gemm=GEMM_3XTF32, max_batch=1, delz=None, lambda_reg=None, relax=None,
+                 flags=0, tc_split_k=0, lsq_method=0, fit_coils=0, sigma_ic=None):
         import torch
         if not torch.cuda.is_available():
             raise PtefitError("no CUDA device: the PTEFIT hot path has no CPU fallback")
         self.torch = torch
         b = dev["basis"]
         self.delz = bool(b.get("delz", 0)) if delz is None else bool(delz)
-        self.terms = poly_terms(b["n_p"], b["n_ff"], self.delz)
+        self.terms = poly_terms(b["n_p"], b["n_ff"], self.delz, b.get("spline"))
         self.prec = PTEFIT_FP32 if precision == "fp32" else PTEFIT_FP64
         self.dtype = torch.float32 if precision == "fp32" else torch.float64
         self.npdtype = np.float32 if precision == "fp32" else np.float64
@@ -173,7 +193,8 @@ class Reconstructor:
         self.max_batch = max_batch
         self.h = ptefit_create(dev["grid"], dev["geom"], dev["tables"], self.terms,
                                b.get("lambda_reg", 0.0) if lambda_reg is None else lambda_reg,
-                               b.get("relax", 1.0) if relax is None else relax, self.prec, gemm, max_batch)
+                               b.get("relax", 1.0) if relax is None else relax, self.prec, gemm, max_batch, flags, tc_split_k,
+                               lsq_method, fit_coils, sigma_ic)
         self.lib = load_library()
         self._alloc(max_batch)
 
@@ -244,11 +265,6 @@ class Reconstructor:
         out = (C.c_float * 6)()
         self._call(self.lib.ptefit_get_stage_ms, out)
         return dict(zip(("setup", "response", "lsq", "boundary", "solve", "search"), list(out)))
-
-    def phase_clocks(self, on=True, read=False):
-        out = (C.c_longlong * 16)() if read else None
-        self._call(self.lib.ptefit_debug_phase_clocks, int(on), out)
-        return list(out) if read else None
 
     def close(self):
         if self.h is not None:

@@ -5,7 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define PTEFIT_MAX_TERMS 12
+#define PTEFIT_MAX_TERMS 16
+#define PTEFIT_MAX_KNOTS 16
 #define PTEFIT_MAX_CAND 32
 #define PTEFIT_MAX_LIM 256
 #define PTEFIT_MAX_NR 257
@@ -15,7 +16,28 @@ namespace ptefit {
 
 constexpr double kMu0 = 1.25663706143591729e-6;  // 4 pi 1e-7 (reading O0)
 
-struct TermDev { int kind, i, N; };
+struct TermDev { int kind, family, i, N; };
+
+// Tension-spline tables (family 1 terms; reading O4c), FP64, in global memory.
+// On [knot_r, knot_r+1], t = (x - knot_r)/h_r:
+//   phi_q = d_qr (1-t) + d_q,r+1 t + m[r][q] (sinh(tau h (1-t))/sinh(tau h) - (1-t))/tau^2 + m[r+1][q] (sinh(tau h t)/sinh(tau h) - t)/tau^2
+struct SplineDev {
+  int nk;
+  double tau, inv_tau2;
+  double knot[PTEFIT_MAX_KNOTS], inv_h[PTEFIT_MAX_KNOTS], tau_h[PTEFIT_MAX_KNOTS], inv_sinh[PTEFIT_MAX_KNOTS];
+  double m[PTEFIT_MAX_KNOTS][PTEFIT_MAX_KNOTS];      // m[r][q] = second derivative of phi_q at knot r
+};
+
+// Caller-owned device pointers of one ptefit_reconstruct call.  The block lives in device memory at a
+// fixed address and is rewritten by k_set_args before every call, so that the captured CUDA graph
+// does not depend on the pointers a caller passes.
+struct CallArgs {
+  const void *b, *ic;
+  void *psi, *coeffs;
+  int *axis_ij; void *axis_rzpsi;
+  int *xpt_ij; void *xpt_rzpsi;
+  void *psi_bnd; int *limited; void *chi2; int *status;
+};
 
 // Per-slice result of the search, kept in double on the device.
 struct SearchOut {
@@ -30,6 +52,10 @@ struct SearchOut {
 template <typename T>
 struct Dev {
   int nr, nz, N, nri, nzi, nbnd, M, nc, nt, npoly, has_delz, nlim, ip_sign;
+  int nspl, maxdeg;               // spline terms among the npoly basis terms; largest polynomial exponent
+  int lsq_method;                 // 0 normal equations + Cholesky, 1 modified Gram-Schmidt
+  const SplineDev *spl;           // nullptr unless nspl > 0
+  const CallArgs *ca;             // device copy of the caller's pointers (k_set_args)
   double rmin, zmin, dr, dz, dA, lambda_reg, relax;
   double cold_rc, cold_zc, cold_a, cold_b;
   TermDev terms[PTEFIT_MAX_TERMS];
@@ -55,7 +81,6 @@ struct Dev {
   double *chi2;                   // [B]
   SearchOut *so;                  // [B]
   int *status;                    // [B]
-  long long *phase_clk;           // [8] optional in-kernel phase timers (ptefit_debug_phase_clocks), else nullptr
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -78,11 +103,37 @@ __device__ __forceinline__ T ipow(T x, int e) {
   return p;
 }
 
+// Cardinal tension spline phi_q(x) (family 1).  Evaluated in FP64 (sinh), x in [0, 1].
+__device__ __forceinline__ double spline_phi(const SplineDev &sp, int q, double x) {
+  if (!(x >= sp.knot[0]) || !(x <= sp.knot[sp.nk - 1])) return 0.0;
+  int r = 0;
+  while (r < sp.nk - 2 && x >= sp.knot[r + 1]) ++r;
+  const double t = fmin(fmax((x - sp.knot[r]) * sp.inv_h[r], 0.0), 1.0), th = sp.tau_h[r];
+  const double A = sinh(th * (1.0 - t)) * sp.inv_sinh[r] - (1.0 - t), Bc = sinh(th * t) * sp.inv_sinh[r] - t;
+  double v = (sp.m[r][q] * A + sp.m[r + 1][q] * Bc) * sp.inv_tau2;
+  if (q == r) v += 1.0 - t;
+  if (q == r + 1) v += t;
+  return v;
+}
+
 template <typename T>
 __device__ __forceinline__ T basis_term(const Dev<T> &D, int l, T x, T rdA, T mu0dA_over_r) {
   const TermDev t = D.terms[l];
-  T v = ipow(x, t.i) - ipow(x, t.N);
-  return (x < T(0)) ? T(0) : v * (t.kind == 0 ? rdA : mu0dA_over_r);
+  if (x < T(0)) return T(0);
+  T v;
+  if (t.family == 1) v = T(spline_phi(*D.spl, t.i, (double)x));
+  else v = ipow(x, t.i) - ipow(x, t.N);
+  return v * (t.kind == 0 ? rdA : mu0dA_over_r);
+}
+
+// Contribution of the spline terms (family 1) to I' = J_b(x) X; the polynomial terms are summed by
+// Horner where this is used.
+template <typename T>
+__device__ __forceinline__ T spline_current(const Dev<T> &D, const double *__restrict__ X, T x, T rdA, T fdA) {
+  T acc = T(0);
+  for (int l = 0; l < D.npoly; ++l)
+    if (D.terms[l].family == 1) acc = fma(basis_term(D, l, x, rdA, fdA), T(X[l]), acc);
+  return acc;
 }
 
 }  // namespace ptefit

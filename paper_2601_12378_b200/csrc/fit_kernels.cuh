@@ -13,6 +13,7 @@ __global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__
   extern __shared__ unsigned char smem_raw[];
   T *sic = reinterpret_cast<T *>(smem_raw);
   const int s = blockIdx.y;
+  if (!b) { b = reinterpret_cast<const T *>(D.ca->b); ic = reinterpret_cast<const T *>(D.ca->ic); }   // graph replay: caller pointers from the argument block
   for (int c = threadIdx.x; c < D.nc; c += blockDim.x) sic[c] = ic[(size_t)s * D.nc + c];
   __syncthreads();
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
@@ -23,11 +24,11 @@ __global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__
     for (int c = 0; c < D.nc; ++c) acc = fma(g[(size_t)c * D.N], sic[c], acc);
     D.psi_coil[(size_t)s * D.N + n] = acc;
   }
-  if (n < D.M) {
-    const T *g = D.gc + (size_t)n * D.nc;
+  for (int m = n; m < D.M; m += gridDim.x * blockDim.x) {       // M may exceed the node count of a small grid
+    const T *g = D.gc + (size_t)m * D.nc;
     T acc = T(0);
     for (int c = 0; c < D.nc; ++c) acc = fma(g[c], sic[c], acc);
-    D.dred[(size_t)s * D.M + n] = b[(size_t)s * D.M + n] - acc;
+    D.dred[(size_t)s * D.M + m] = b[(size_t)s * D.M + m] - acc;
   }
   if (n < D.nt) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
   if (n == 0) { D.status[s] = 0; D.chi2[s] = 0.0; }

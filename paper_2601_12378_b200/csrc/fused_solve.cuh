@@ -38,16 +38,18 @@ __device__ __forceinline__ Vec2<double> load2(const double *p) {
 
 // Shared-memory bytes of k_solve_fused for a grid (host and device agree through this).
 template <typename T>
-__host__ __device__ inline size_t fused_smem_bytes(int nr, int nz, bool pre = false) {
+__host__ __device__ inline size_t fused_smem_bytes(int nr, int nz) {
   const int n2 = (nz - 1) / 2;
   const size_t g = ((size_t)nz * nr + 3) & ~(size_t)3;          // 16-byte aligned sub-arrays
-  size_t e = pre ? 0 : 2 * (size_t)n2 * FUSED_CW * sizeof(T);     // fold buffer, reused for the bit masks
+  size_t e = 2 * (size_t)n2 * FUSED_CW * sizeof(T);              // fold buffer, reused for the bit masks
   const size_t mb = 3 * (((size_t)nz * nr + 31) / 32) * sizeof(unsigned);   // lim, xpt, edge bit masks
   if (mb > e) e = mb;
   const size_t pbb = (size_t)(2 * (nr + nz) - 4) * sizeof(T);   // ... and for the boundary flux
   if (pbb > e) e = pbb;
+  const size_t exb = 2 * (size_t)(FUSED_THREADS / 2) * sizeof(double);   // ... and for the twisted-Thomas hand-over
+  if (exb > e) e = exb;
   e = (e + 15) & ~(size_t)15;
-  return (g + (pre ? 0 : 2 * (size_t)n2 * n2)) * sizeof(T) + e;
+  return (g + 2 * (size_t)n2 * n2) * sizeof(T) + e;
 }
 
 // In-place DST-I along Z of the interior columns of G[nz][nr] (rows 1..nz-2 <-> modes 1..nz-2),
@@ -104,8 +106,6 @@ __device__ void dst_columns(T *G, const T *So, const T *Se, T *E, int nr, int nz
   }
 }
 
-// Optional phase timers (D.phase_clk != nullptr): thread 0 of CTA 0 accumulates clock64 deltas.
-#define PTEFIT_PHASE(k) do { if (D.phase_clk && tid == 0 && blockIdx.x == 0) { const long long t_ = clock64(); D.phase_clk[k] += t_ - t_phase; t_phase = t_; } } while (0)
 
 __device__ __forceinline__ void cp_async4(void *smem, const void *gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
@@ -121,24 +121,22 @@ __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefe
 // grid min(B, resident CTAs), block FUSED_THREADS, dyn smem fused_smem_bytes<T>(nr, nz).
 // cur[B][N] node currents (A), pbd[B][nbnd] boundary flux, psi[B][N] in/out.
 // do_search = 0: Delta* solve only (debug hook); 1: also search + xn (+ dzc when has_delz).
-// pl_all != nullptr: the plasma flux of the interior nodes was already solved (split_solve.cuh):
-// load it instead of the currents and skip the solve phases.
-template <typename T, bool PRE = false>
+template <typename T>
 __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int B, const T *__restrict__ cur_all,
                                                                 const T *__restrict__ pbd_all, T *__restrict__ psi_all,
                                                                 T *__restrict__ xn_all, int use_relax, int add_coil,
-                                                                int do_search, const T *__restrict__ pl_all) {
+                                                                int do_search) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  if (!psi_all) psi_all = reinterpret_cast<T *>(D.ca->psi);
   const int nr = D.nr, nz = D.nz, N = D.N, nri = D.nri, nzi = D.nzi, Nz = nz - 1, n2 = Nz / 2;
   const int tid = threadIdx.x, nth = blockDim.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
   T *G = reinterpret_cast<T *>(smem_raw);
   T *So = G + ((N + 3) & ~3);
   T *Se = So + n2 * n2;
-  T *E = PRE ? So : Se + n2 * n2;                          // PRE: no DST tables in shared memory
+  T *E = Se + n2 * n2;
   unsigned *mbits = reinterpret_cast<unsigned *>(E);        // during the search: lim bits, then xpt bits
   const int nwords = (N + 31) >> 5;
-  if (!PRE)
-    for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];    // So then Se, contiguous
+  for (int e = tid; e < 2 * n2 * n2; e += nth) So[e] = D.dst_tab[e];    // So then Se, contiguous
   // per-column constants (same expressions as the unfused kernels, evaluated once per CTA)
   __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
   __shared__ T pcoef[2 * (PTEFIT_MAX_DEG + 1)];              // I'(x) = rdA P(x) + fdA Q(x)
@@ -154,10 +152,9 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
   }
   const T cz = T(1.0 / (D.dz * D.dz));
   const T scale = T(2.0 / Nz);
-  const T esc = pl_all ? T(1) : scale;             // the split path stores the flux already scaled
+  const T esc = scale;
   const T om = T(D.relax);
   const double sg = (double)D.ip_sign;
-  long long t_phase = clock64();
   for (int s = blockIdx.x; s < B; s += gridDim.x) {
     const T *I = cur_all + (size_t)s * N;
     const T *pbg = pbd_all + (size_t)s * D.nbnd;          // bottom[nr], top[nr], left[nzi], right[nzi]
@@ -168,8 +165,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
     // ---- node currents straight into shared memory (asynchronous copies, no register staging)
     for (int k = tid; k < D.nbnd; k += nth) E[k] = pbg[k];
     for (int n = tid; n < N; n += nth) {
-      const T *src = pl_all ? pl_all + (size_t)s * N + n : I + n;
-      if (sizeof(T) == 4) cp_async4(G + n, src); else cp_async8(G + n, src);
+      if (sizeof(T) == 4) cp_async4(G + n, I + n); else cp_async8(G + n, I + n);
     }
     // inputs of the later phases: pull them into L2 while the solve runs
     {
@@ -185,24 +181,12 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
       const double *Xp = D.X + (size_t)s * D.nt;
       double c = 0.0;
       for (int l = 0; l < D.npoly; ++l)
-        if (D.terms[l].kind == kind) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+        if (D.terms[l].kind == kind && D.terms[l].family == 0) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
       pcoef[tid] = T(c);
     }
-    PTEFIT_PHASE(14);
     cp_async_wait_all();
     __syncthreads();
-    PTEFIT_PHASE(15);
-    if (PRE || pl_all) {                                   // solved elsewhere: only the edge data is missing
-      for (int k = tid; k < D.nbnd; k += nth) {
-        int n;
-        if (k < nr) n = k;
-        else if (k < 2 * nr) n = (nz - 1) * nr + (k - nr);
-        else if (k < 2 * nr + nzi) n = (k - 2 * nr + 1) * nr;
-        else n = (k - 2 * nr - nzi + 1) * nr + nr - 1;
-        G[n] = pb[k];
-      }
-      __syncthreads();
-    } else {
+    {
     // ---- right-hand side -mu0 R I / dA with the Dirichlet data moved over (interior), edge data (edges)
     // (one warp per grid row: the row tests are warp-uniform, the column tests plain selects)
     for (int j = warp; j < nz; j += nwarp) {
@@ -226,9 +210,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
       }
     }
     __syncthreads();
-    PTEFIT_PHASE(0);
     dst_columns<T>(G, So, Se, E, nr, nz);
-    PTEFIT_PHASE(1);
     // ---- Thomas sweeps along R in FP64, one thread per mode (precomputed factors).
     // The dependent chain is one DFMA per step.
     if (2 * nzi <= nth && nri >= 3) {
@@ -333,9 +315,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
       }
     }
     __syncthreads();
-    PTEFIT_PHASE(2);
     dst_columns<T>(G, So, Se, E, nr, nz);
-    PTEFIT_PHASE(3);
     }
     // ---- bit masks of the search into the (now free) fold buffer
     for (int w = tid; w < 3 * nwords; w += nth)
@@ -385,14 +365,12 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
       so_opt.am.n = am_n;
     }
     __syncthreads();
-    PTEFIT_PHASE(4);
     if (do_search) {
       T *xn = xn_all + (size_t)s * N;
       so_opt.lbits = mbits; so_opt.xbits = mbits + nwords; so_opt.have_am = true;
       so_opt.local = G;
-      if (D.has_delz) { so_opt.pc = pcoef; so_opt.rdA = c_rdA; so_opt.fdA = c_fdA; }
+      if (D.has_delz) { so_opt.pc = pcoef; so_opt.rdA = c_rdA; so_opt.fdA = c_fdA; so_opt.Xs = D.X + (size_t)s * D.nt; }
       search_body<T>(D, s, G, xn, so_opt);                 // G now holds I'(xn) (delz) or xn
-      PTEFIT_PHASE(5);
       if (D.has_delz) {
         // -dI'/dZ column for the NEXT fit (I' = J_b(xn) X with the coefficients of this fit)
         __syncthreads();
@@ -406,7 +384,6 @@ __global__ void __launch_bounds__(FUSED_THREADS, 2) k_solve_fused(Dev<T> D, int 
           dzc[n] = edge ? T(0) : -(G[up] - G[dn]) * hz;
         }
       }
-      PTEFIT_PHASE(6);
     }
   }
 }

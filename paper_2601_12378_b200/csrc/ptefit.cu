@@ -18,13 +18,13 @@
 #include "fused_solve.cuh"
 #include "tc_gemm.cuh"
 #include "tc_kernels.cuh"
-#include "split_solve.cuh"
+#include "tc_solve.cuh"
 
 using namespace ptefit;
 
 static thread_local std::string g_error;
 
-struct GraphKey { int batch, n_iter, warm; const void *p[13]; };
+struct GraphKey { int batch, n_iter, warm; };
 struct CachedGraph { GraphKey key; cudaGraphExec_t exec; int launches; };
 
 struct ptefit_handle {
@@ -39,23 +39,23 @@ struct ptefit_handle {
   bool tc = false;                      // tensor-core contractions usable (FP32, 3xTF32 mode)
   TcDev Tc{};
   const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;
-  int pbd_ntiles = 0;
+  int pbd_ntiles = 0, max_split_resp = 1, max_split_pbd = 1;
   const float *c_rdA = nullptr, *c_fdA = nullptr;   // Eq. 10 factors on the compact node list
-  bool split = false;                   // solve as batched DST GEMMs + tridiagonal kernel (PTEFIT_SPLIT_SOLVE)
-  SplitDev Sp{};
-  const float *s_hi = nullptr, *s_lo = nullptr;
-  CUtensorMap mapSaHi, mapSaLo, mapSxHi, mapSxLo, mapSHi, mapSLo;
+  bool tcs = false;                     // k_solve_tc usable (FP32, N_Z = 129, tensor-core mode)
+  TcSolveDev Ts{};
+  size_t tcs_smem = 0;
+  int nsm = 0;
+  CUtensorMap mapTfHi, mapTfLo, mapTiHi, mapTiLo;   // forward / inverse sine tables of k_solve_tc
+  int flags = 0, tc_split_k = 0;
+  CallArgs *ca_dev = nullptr;           // device copy of the caller's pointers, rewritten per call
   int std_np = 0;                       // > 0: standard term list, basis generated inside the response GEMM
   CUtensorMap mapJbHi, mapJbLo, mapGpHi, mapGpLo, mapCurHi, mapCurLo, mapGbHi, mapGbLo;
-  long long *phase_clk = nullptr;       // device, ptefit_debug_phase_clocks
-  bool use_graph = true;                // replay the launch sequence as a CUDA graph (PTEFIT_NO_GRAPH=1 disables)
+  bool use_graph = true;                // replay the launch sequence as a CUDA graph (PTEFIT_OPT_NO_GRAPH disables)
   std::vector<CachedGraph> graphs;
   cudaStream_t gstream = nullptr;       // capture stream
   bool fused = false;                   // k_solve_fused usable (slice fits shared memory)
   int fused_grid = 0;                   // resident CTAs of k_solve_fused
   size_t fused_smem = 0;
-  int fused_pre_grid = 0;               // lean variant of k_solve_fused used by the split solve path
-  size_t fused_pre_smem = 0;
   bool profiling = false;
   std::vector<cudaEvent_t> ev;          // stage boundaries of the last call
   std::vector<int> ev_stage;
@@ -122,11 +122,51 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   D.dr = (g->rmax - g->rmin) / (g->nr - 1); D.dz = (g->zmax - g->zmin) / (g->nz - 1);
   D.dA = D.dr * D.dz; D.lambda_reg = ba->lambda_reg; D.relax = ba->relax;
   D.cold_rc = ge->cold_rc; D.cold_zc = ge->cold_zc; D.cold_a = ge->cold_a; D.cold_b = ge->cold_b;
-  D.npoly = 0; D.has_delz = 0; D.phase_clk = nullptr;
+  D.npoly = 0; D.has_delz = 0; D.nspl = 0; D.maxdeg = 0; D.spl = nullptr; D.lsq_method = ba->lsq_method;
+  const ptefit_term *spl_term = nullptr;
   for (int l = 0; l < ba->n_terms; ++l) {
-    D.terms[l].kind = ba->terms[l].kind; D.terms[l].i = ba->terms[l].i; D.terms[l].N = ba->terms[l].N;
-    if (ba->terms[l].kind == 2) D.has_delz = 1; else D.npoly++;
+    const ptefit_term &t = ba->terms[l];
+    D.terms[l].kind = t.kind; D.terms[l].family = t.kind == 2 ? 0 : t.family; D.terms[l].i = t.i; D.terms[l].N = t.N;
+    if (t.kind == 2) { D.has_delz = 1; continue; }
+    D.npoly++;
+    if (t.family == 1) { D.nspl++; spl_term = &t; }
+    else if (t.N > D.maxdeg) D.maxdeg = t.N;
   }
+  if (spl_term) {
+    // cardinal tension splines (reading O4c): second derivatives m[r][q] at the knots from the
+    // tridiagonal system that makes the first derivative continuous (natural ends), solved in FP64
+    SplineDev sp{};
+    const int nk = spl_term->n_knots;
+    const double tau = spl_term->tension;
+    sp.nk = nk; sp.tau = tau; sp.inv_tau2 = 1.0 / (tau * tau);
+    std::vector<double> a(nk, 0.0), b(nk, 0.0);
+    for (int r = 0; r < nk; ++r) sp.knot[r] = spl_term->knots[r];
+    for (int r = 0; r + 1 < nk; ++r) {
+      const double hh = sp.knot[r + 1] - sp.knot[r];
+      sp.inv_h[r] = 1.0 / hh; sp.tau_h[r] = tau * hh; sp.inv_sinh[r] = 1.0 / sinh(tau * hh);
+      a[r] = (1.0 / hh - tau / sinh(tau * hh)) / (tau * tau);
+      b[r] = (tau * cosh(tau * hh) / sinh(tau * hh) - 1.0 / hh) / (tau * tau);
+    }
+    for (int q = 0; q < nk; ++q) {                       // one Thomas solve per cardinal function
+      std::vector<double> lo(nk, 0.0), di(nk, 1.0), up(nk, 0.0), rh(nk, 0.0);
+      for (int r = 1; r + 1 < nk; ++r) {
+        lo[r] = a[r - 1]; di[r] = b[r - 1] + b[r]; up[r] = a[r];
+        const double y0 = (r - 1 == q), y1 = (r == q), y2 = (r + 1 == q);
+        rh[r] = (y2 - y1) * sp.inv_h[r] - (y1 - y0) * sp.inv_h[r - 1];
+      }
+      for (int r = 1; r < nk; ++r) { const double w = lo[r] / di[r - 1]; di[r] -= w * up[r - 1]; rh[r] -= w * rh[r - 1]; }
+      std::vector<double> mm(nk, 0.0);
+      mm[nk - 1] = rh[nk - 1] / di[nk - 1];
+      for (int r = nk - 2; r >= 0; --r) mm[r] = (rh[r] - up[r] * mm[r + 1]) / di[r];
+      for (int r = 0; r < nk; ++r) sp.m[r][q] = mm[r];
+    }
+    SplineDev *dsp = nullptr;
+    TRY(dev_alloc(h, &dsp, 1));
+    CK(cudaMemcpy(dsp, &sp, sizeof sp, cudaMemcpyHostToDevice));
+    D.spl = dsp;
+  }
+  TRY(dev_alloc(h, &h->ca_dev, 1));
+  D.ca = h->ca_dev;
   const size_t N = D.N;
   // tables; edge-node columns of gp / gb are zeroed (edge nodes never carry current)
   {
@@ -290,13 +330,37 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
           return fail(h, PTEFIT_ERR_INVALID_ARG, "lim_mask / xpt_mask must be 0 on edge nodes");
       }
   if (!tb->gp || !tb->gc || !tb->gb || !tb->ggc) return fail(h, PTEFIT_ERR_INVALID_ARG, "null table");
-  if (ba->n_terms < 1 || ba->n_terms > PTEFIT_MAX_TERMS || !ba->terms) return fail(h, PTEFIT_ERR_INVALID_ARG, "n_terms must be in [1,12]");
-  for (int l = 0; l < ba->n_terms; ++l) {
-    const ptefit_term &t = ba->terms[l];
-    if (t.kind < 0 || t.kind > 2) return fail(h, PTEFIT_ERR_UNSUPPORTED, "unknown basis term kind");
-    if (t.kind == 2 && l != ba->n_terms - 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "the vertical-shift term must be last");
-    if (t.kind != 2 && (t.i < 0 || t.N <= t.i || t.N > 8)) return fail(h, PTEFIT_ERR_INVALID_ARG, "term exponents need 0 <= i < N <= 8");
+  if (ba->n_terms < 1 || ba->n_terms > PTEFIT_MAX_TERMS || !ba->terms) return fail(h, PTEFIT_ERR_INVALID_ARG, "n_terms must be in [1,16]");
+  {
+    const ptefit_term *sp0 = nullptr;
+    for (int l = 0; l < ba->n_terms; ++l) {
+      const ptefit_term &t = ba->terms[l];
+      if (t.kind < 0 || t.kind > 2) return fail(h, PTEFIT_ERR_UNSUPPORTED, "unknown basis term kind");
+      if (t.kind == 2 && l != ba->n_terms - 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "the vertical-shift term must be last");
+      if (t.kind == 2) continue;
+      if (t.family < 0 || t.family > 1) return fail(h, PTEFIT_ERR_UNSUPPORTED, "unknown basis term family");
+      if (t.family == 0 && (t.i < 0 || t.N <= t.i || t.N > 8)) return fail(h, PTEFIT_ERR_INVALID_ARG, "term exponents need 0 <= i < N <= 8");
+      if (t.family == 1) {
+        if (t.n_knots < 3 || t.n_knots > PTEFIT_MAX_KNOTS || !t.knots || !(t.tension > 0.0) || t.i < 0 || t.i >= t.n_knots)
+          return fail(h, PTEFIT_ERR_INVALID_ARG, "spline term needs 3..16 knots, tension > 0 and 0 <= i < n_knots");
+        for (int r = 0; r + 1 < t.n_knots; ++r)
+          if (!(t.knots[r + 1] > t.knots[r])) return fail(h, PTEFIT_ERR_INVALID_ARG, "spline knots must be strictly increasing");
+        if (sp0 && (sp0->n_knots != t.n_knots || sp0->tension != t.tension || memcmp(sp0->knots, t.knots, sizeof(double) * t.n_knots) != 0))
+          return fail(h, PTEFIT_ERR_UNSUPPORTED, "all spline terms must share one knot set and tension");
+        sp0 = &t;
+      }
+    }
   }
+  if (ba->lsq_method != 0 && ba->lsq_method != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "lsq_method must be 0 (normal equations) or 1 (Gram-Schmidt QR)");
+  if (ba->fit_coils != 0 && ba->fit_coils != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils must be 0 or 1");
+  if (ba->fit_coils) {
+    if (!ba->sigma_ic) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils needs sigma_ic");
+    for (int c = 0; c < ge->n_coil; ++c)
+      if (!(ba->sigma_ic[c] > 0.0)) return fail(h, PTEFIT_ERR_INVALID_ARG, "sigma_ic must be > 0");
+  }
+  if (op->gemm != PTEFIT_GEMM_3XTF32 && op->gemm != PTEFIT_GEMM_FFMA) return fail(h, PTEFIT_ERR_INVALID_ARG, "gemm must be PTEFIT_GEMM_3XTF32 or PTEFIT_GEMM_FFMA");
+  if (op->flags & ~(PTEFIT_OPT_NO_GRAPH | PTEFIT_OPT_NO_FUSED_BASIS | PTEFIT_OPT_SOLVE_FFMA)) return fail(h, PTEFIT_ERR_INVALID_ARG, "unknown option flag");
+  if (op->tc_split_k < 0) return fail(h, PTEFIT_ERR_INVALID_ARG, "tc_split_k must be >= 0");
   if (ba->n_terms == 1 && ba->terms[0].kind == 2) return fail(h, PTEFIT_ERR_INVALID_ARG, "need at least one P'/FF' term");
   if (!(ba->lambda_reg >= 0.0) || !(ba->relax > 0.0) || ba->relax > 1.0) return fail(h, PTEFIT_ERR_INVALID_ARG, "need lambda_reg >= 0 and 0 < relax <= 1");
   if (op->max_batch < 1 || op->max_batch > 65535) return fail(h, PTEFIT_ERR_INVALID_ARG, "max_batch must be in [1,65535]");
@@ -311,10 +375,12 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   }
   h = new ptefit_handle();
   h->prec = op->precision; h->gemm = op->gemm; h->max_batch = op->max_batch;
-  h->use_graph = getenv("PTEFIT_NO_GRAPH") == nullptr;
+  h->flags = op->flags; h->tc_split_k = op->tc_split_k;
+  h->use_graph = !(op->flags & PTEFIT_OPT_NO_GRAPH);
+  { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->nsm, cudaDevAttrMultiProcessorCount, dev); }
   ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
                                               : build(h, h->d64, g, ge, tb, ba, op->max_batch);
-  if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) { st = build_tc(h, h->d32, ge, tb, op->max_batch); if (st == PTEFIT_OK) st = build_split(h, h->d32, op->max_batch); }
+  if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) { st = build_tc(h, h->d32, ge, tb, op->max_batch); if (st == PTEFIT_OK) st = build_tcsolve(h, h->d32); }
   if (st != PTEFIT_OK) { std::string e = h->error; ptefit_destroy(h); g_error = e; return st; }
   *out = h;
   return PTEFIT_OK;
@@ -328,7 +394,6 @@ extern "C" void ptefit_destroy(ptefit_handle *h) {
   for (void *p : hp) if (p) cudaFree(p);
   for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
   if (h->gstream) cudaStreamDestroy(h->gstream);
-  if (h->phase_clk) cudaFree(h->phase_clk);
   if (h->hstream) cudaStreamDestroy(h->hstream);
   delete h;
 }

@@ -75,6 +75,7 @@ struct SearchOpt {
   T *local = nullptr;                // per-node output in shared memory (may alias psi)
   const T *pc = nullptr;             // if set: local gets I'(xn) = rdA P(xn) + fdA Q(xn) instead of xn
   const T *rdA = nullptr, *fdA = nullptr;
+  const double *Xs = nullptr;        // coefficients of this slice (spline terms of I', if any)
 };
 
 // Search of one slice by one CTA (any block size that is a multiple of 32, <= 1024).  Reads
@@ -82,7 +83,6 @@ struct SearchOpt {
 // global memory and, if o.local != nullptr, a per-node value to o.local (may alias psi: every
 // thread overwrites only nodes it alone reads after the last barrier).  Updates D.so[s],
 // D.status[s] (sticky).  All threads of the CTA must call it.
-#define PTEFIT_SP(k) do { if (D.phase_clk && threadIdx.x == 0 && blockIdx.x == 0) { const long long t_ = clock64(); D.phase_clk[k] += t_ - t_sp; t_sp = t_; } } while (0)
 
 template <typename T>
 __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict__ xn, const SearchOpt<T> &o) {
@@ -94,7 +94,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   __shared__ double cR[PTEFIT_MAX_CAND], cZ[PTEFIT_MAX_CAND], cP[PTEFIT_MAX_CAND];
   __shared__ int cN[PTEFIT_MAX_CAND];
   __shared__ SearchOut so;
-  long long t_sp = clock64();
   if (tid == 0) { sh_flag = 0; sh_ncand = 0; sh_count = 0; }
   __syncthreads();
   // 0. finiteness + 1. axis node: arg-max of s*psi over lim_mask, tie -> smallest n
@@ -113,7 +112,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   }
   if (bad) atomicOr(&sh_flag, 1);
   am = block_argmax(am, sh_am);
-  PTEFIT_SP(8);
   int status = 0;
   if (sh_flag) status = 2;
   double Ra = 0, Za = 0, Pa = 0;
@@ -124,7 +122,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     if (!(f.det > 0.0) || fmax(fabs(f.xs), fabs(f.ys)) > 1.0) status = 1;
     Ra = D.rmin + (ia + f.xs) * D.dr; Za = D.zmin + (ja + f.ys) * D.dz; Pa = f.ps;
   }
-  PTEFIT_SP(9);
   // 2. X-point candidates (det H < 0, stationary point inside the half cell, below the axis flux)
   if (status == 0) {
     for (int j = warp + 1; j < nz - 1; j += nwarp)
@@ -167,7 +164,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
   }
   __syncthreads();
-  PTEFIT_SP(10);
   const int ncand = sh_ncand;
   if (status == 0 && ncand > PTEFIT_MAX_CAND) status = 4;
   // 3. limiter vertices: bilinear flux, valid iff not behind any candidate as seen from the axis
@@ -189,7 +185,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
   }
   lm = block_argmax(lm, sh_am);
-  PTEFIT_SP(11);
   // 4. boundary flux
   double Pb = 0.0;
   if (status == 0) {
@@ -215,7 +210,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
     }
     if (Pb == Pa) status = 1;
   }
-  PTEFIT_SP(12);
   // 5./6. plasma region and normalised flux
   int cnt = 0;
   if (status == 0) {
@@ -251,6 +245,7 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
             hq = fma(hq, out, pco[PTEFIT_MAX_DEG + 1 + k]);
           }
           lv = (out < T(0)) ? T(0) : fma(o.rdA[i], hp, o.fdA[i] * hq);
+          if (D.nspl && o.Xs) lv += spline_current(D, o.Xs, out, o.rdA[i], o.fdA[i]);
         }
         o.local[n] = lv;
       }
@@ -263,7 +258,6 @@ __device__ void search_body(const Dev<T> &D, int s, const T *psi, T *__restrict_
   }
   if (cnt) atomicAdd(&sh_count, cnt);
   __syncthreads();
-  PTEFIT_SP(13);
   if (status == 0 && sh_count == 0) status = 1;
   if (tid == 0) {
     if (D.status[s] == 0) {
@@ -279,6 +273,7 @@ template <typename T>
 __global__ void __launch_bounds__(SEARCH_THREADS) k_search(Dev<T> D, const T *__restrict__ psi_all,
                                                             T *__restrict__ xn_all) {
   const int s = blockIdx.x;
+  if (!psi_all) psi_all = reinterpret_cast<const T *>(D.ca->psi);
   SearchOpt<T> o;
   search_body<T>(D, s, psi_all + (size_t)s * D.N, xn_all + (size_t)s * D.N, o);
 }
@@ -289,6 +284,12 @@ __global__ void k_export(Dev<T> D, int B, T *coeffs, int *axis_ij, T *axis_rzpsi
                          T *xpt_rzpsi, T *psi_bnd, int *limited, T *chi2, int *status) {
   const int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= B) return;
+  if (!coeffs && !axis_ij && !status && !chi2 && !psi_bnd) {     // graph replay: caller pointers from the argument block
+    const CallArgs a = *D.ca;
+    coeffs = reinterpret_cast<T *>(a.coeffs); axis_ij = a.axis_ij; axis_rzpsi = reinterpret_cast<T *>(a.axis_rzpsi);
+    xpt_ij = a.xpt_ij; xpt_rzpsi = reinterpret_cast<T *>(a.xpt_rzpsi); psi_bnd = reinterpret_cast<T *>(a.psi_bnd);
+    limited = a.limited; chi2 = reinterpret_cast<T *>(a.chi2); status = a.status;
+  }
   const SearchOut o = D.so[s];
   if (coeffs) for (int l = 0; l < D.nt; ++l) coeffs[(size_t)s * D.nt + l] = T(D.X[(size_t)s * D.nt + l]);
   if (axis_ij) { axis_ij[2 * s] = o.axis_i; axis_ij[2 * s + 1] = o.axis_j; }

@@ -83,6 +83,7 @@ template <typename T>
 __global__ void __launch_bounds__(DST_THREADS) k_idst_total(Dev<T> D, T *__restrict__ psi, int use_relax,
                                                              int add_coil) {
   extern __shared__ unsigned char smem_raw[];
+  if (!psi) psi = reinterpret_cast<T *>(D.ca->psi);
   T *f = reinterpret_cast<T *>(smem_raw);          // [DST_COLS][nzi+1]
   const int s = blockIdx.y, i0 = 1 + blockIdx.x * DST_COLS;
   const int nr = D.nr, nz = D.nz, nri = D.nri, nzi = D.nzi, ld = nzi + 1;
@@ -121,6 +122,7 @@ __global__ void k_edge_total(Dev<T> D, T *__restrict__ psi, const T *__restrict_
                              int add_coil) {
   const int s = blockIdx.y, k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= D.nbnd) return;
+  if (!psi) psi = reinterpret_cast<T *>(D.ca->psi);
   const int nr = D.nr, nz = D.nz, nzi = D.nzi;
   int n;
   if (k < nr) n = k;

@@ -51,6 +51,7 @@ __global__ void __launch_bounds__(128) k_basis_split(Dev<float> D, TcDev Tc) {
 #pragma unroll
       for (int k = 0; k <= PTEFIT_MAX_DEG; ++k) { a = (k == t.i) ? pw[k] : a; b = (k == t.N) ? pw[k] : b; }
       v = (x < 0.f) ? 0.f : (a - b) * (t.kind == 0 ? rdA : fdA);
+      if (t.family == 1) v = basis_term(D, l, x, rdA, fdA);
     } else {
       v = D.dzc[(size_t)s * D.N + n];
     }
@@ -84,7 +85,7 @@ __global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
     const int kind = threadIdx.x / (PTEFIT_MAX_DEG + 1), k = threadIdx.x - kind * (PTEFIT_MAX_DEG + 1);
     double c = 0.0;
     for (int l = 0; l < D.npoly; ++l)
-      if (D.terms[l].kind == kind) c += X[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+      if (D.terms[l].kind == kind && D.terms[l].family == 0) c += X[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
     pco[threadIdx.x] = float(c);
   }
   if (threadIdx.x == 32) xdz = D.has_delz ? float(X[D.nt - 1]) : 0.f;
@@ -104,6 +105,7 @@ __global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
 #pragma unroll
     for (int k = PTEFIT_MAX_DEG - 1; k >= 0; --k) { hp = fmaf(hp, x, cp[k]); hq = fmaf(hq, x, cp[PTEFIT_MAX_DEG + 1 + k]); }
     float v = (x < 0.f) ? 0.f : fmaf(rdA, hp, fdA * hq);
+    if (D.nspl) v += spline_current(D, X, x, rdA, fdA);
     if (D.has_delz) v = fmaf(D.dzc[(size_t)s * D.N + n], xd, v);
     if (n != 0) D.cur[(size_t)s * D.N + n] = v;        // padding entries point at node 0
     const float hi = tf32_rna(v);

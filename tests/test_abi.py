@@ -74,9 +74,12 @@ def _create_status(d, terms=None, **over):
                       geom["cold_zc"], geom["cold_a"], geom["cold_b"])
     tb = Bd._Tables(Bd._ptr(keep["gp"]), Bd._ptr(keep["gc"]), Bd._ptr(keep["gb"]), Bd._ptr(keep["ggc"]))
     terms = terms if terms is not None else P.poly_terms(2, 2, True)
-    tarr = (Bd._Term * len(terms))(*[Bd._Term(*t) for t in terms])
-    ba = Bd._Basis(len(terms), tarr, float(over.get("lambda_reg", 0.01)), float(over.get("relax", 0.6)))
-    op = Bd._Options(int(over.get("precision", 1)), 0, int(over.get("max_batch", 1)))
+    kk = []
+    tarr = (Bd._Term * len(terms))(*[Bd._term_struct(t, kk) for t in terms])
+    ba = Bd._Basis(len(terms), tarr, float(over.get("lambda_reg", 0.01)), float(over.get("relax", 0.6)),
+                   int(over.get("lsq_method", 0)), int(over.get("fit_coils", 0)), None)
+    op = Bd._Options(int(over.get("precision", 1)), int(over.get("gemm", 0)), int(over.get("max_batch", 1)),
+                     int(over.get("flags", 0)), 0)
     h = C.c_void_p()
     st = lib.ptefit_create(C.byref(g), C.byref(ge), C.byref(tb), C.byref(ba), C.byref(op), C.byref(h))
     msg = lib.ptefit_global_error().decode()
@@ -109,3 +112,12 @@ def test_create_validates_arguments_on_the_host():
     assert _create_status(d, terms=[(0, 2, 2)])[0] == INVALID                           # needs i < N
     assert _create_status(d, terms=[(5, 0, 2)])[0] == UNSUPPORTED                       # unknown kind
     assert _create_status(d, terms=[(2, 0, 0)])[0] == INVALID                           # no P'/FF' term at all
+    kn = np.linspace(0.7, 1.0, 7)
+    assert _create_status(d, terms=[(0, 0, 1), (1, 9, 0, 1, kn, 10.0)])[0] == INVALID     # cardinal index out of range
+    assert _create_status(d, terms=[(0, 0, 1), (1, 2, 0, 1, kn[::-1], 10.0)])[0] == INVALID   # knots must increase
+    assert _create_status(d, terms=[(0, 0, 1), (1, 2, 0, 1, kn, 0.0)])[0] == INVALID      # tension > 0
+    assert _create_status(d, terms=[(0, 0, 1), (1, 2, 0, 1, kn, 10.0), (1, 3, 0, 1, kn, 5.0)])[0] == UNSUPPORTED   # one tension only
+    assert _create_status(d, gemm=1)[0] == INVALID                                       # reserved single-pass TF32 mode
+    assert _create_status(d, flags=64)[0] == INVALID
+    assert _create_status(d, lsq_method=2)[0] == INVALID
+    assert _create_status(d, fit_coils=1)[0] == INVALID                                  # needs sigma_ic

@@ -232,29 +232,31 @@ def test_paper_form_without_additions():
     rec.close()
 
 
-@pytest.mark.parametrize("variant", ["ffma", "nonstandard_terms", "no_graph_profiling", "split_solve"])
+@pytest.mark.parametrize("variant", ["ffma", "nonstandard_terms", "no_graph_profiling", "solve_ffma_129", "no_fused_basis", "spline_terms"])
 def test_fp32_code_path_variants(variant):
-    """The FP32 path has three contraction routes (and an opt-in split Delta* solve): tcgen05 GEMM with in-kernel basis producer (the
-    default, covered above), tcgen05 GEMM fed by k_basis_split (term lists that are not NP = NFF in
-    {2, 3}), and the plain FMA kernels (PTEFIT_GEMM_FFMA).  Each must meet the same tolerances; the
-    stage-event (non-graph) launch path must give bit-identical results to the graph replay."""
+    """The FP32 path has three contraction routes and two Delta* solve routes: tcgen05 GEMM with
+    in-kernel basis producer (the default, covered above), tcgen05 GEMM fed by k_basis_split (term
+    lists that are not NP = NFF in {2, 3}, spline terms, or PTEFIT_OPT_NO_FUSED_BASIS), the plain FMA
+    kernels (PTEFIT_GEMM_FFMA); k_solve_tc (129-row grids, default) and k_solve_fused
+    (PTEFIT_OPT_SOLVE_FFMA and all other grids).  Each must meet the same tolerances; the stage-event
+    (non-graph) launch path must give bit-identical results to the graph replay."""
     torch = _torch()
     import paper_2601_12378_b200 as P
-    from paper_2601_12378_b200.binding import GEMM_FFMA
-    import os
-    dev, sl = cached_case("cfg3" if variant == "split_solve" else "cfg2", 2)
-    if variant == "split_solve":      # opt-in path: Delta* solve as batched DST GEMMs + tridiagonal kernel
-        os.environ["PTEFIT_SPLIT_SOLVE"] = "1"
+    from paper_2601_12378_b200.binding import GEMM_FFMA, OPT_SOLVE_FFMA, OPT_NO_FUSED_BASIS
+    dev, sl = cached_case("cfg3" if variant == "solve_ffma_129" else "cfg2", 2)
     if variant == "nonstandard_terms":
         dev = dict(dev); dev["basis"] = dict(dev["basis"], n_p=3, n_ff=2)
+    if variant == "spline_terms":
+        dev = dict(dev); dev["basis"] = dict(dev["basis"], n_p=2, n_ff=2, spline=dict(knots=np.linspace(0.7, 1.0, 7), tension=10.0, terms=[2, 4]))
     dv, b, ic = round_inputs(dev, sl, "fp32")
     od = oracle_device(dv)
     n_iter = 8
     kw = dict(gemm=GEMM_FFMA) if variant == "ffma" else {}
-    try:
-        rec = _rec(dev, "fp32", 2, **kw)
-    finally:
-        os.environ.pop("PTEFIT_SPLIT_SOLVE", None)
+    if variant == "solve_ffma_129":
+        kw = dict(flags=OPT_SOLVE_FFMA)
+    if variant == "no_fused_basis":
+        kw = dict(flags=OPT_NO_FUSED_BASIS)
+    rec = _rec(dev, "fp32", 2, **kw)
     db = torch.tensor(b, dtype=rec.dtype, device="cuda"); dic = torch.tensor(ic, dtype=rec.dtype, device="cuda")
     rec.reconstruct(db, dic, n_iter)
     torch.cuda.synchronize()
