@@ -66,7 +66,11 @@ struct Dev {
   const uint8_t *lim_mask, *xpt_mask;
   const unsigned *lim_bits, *xpt_bits;   // the same masks bit-packed: bit (n & 31) of word n >> 5
   const unsigned *edge_bits;             // bit set for the nodes of the grid edge
+  const unsigned *dil_bits;              // lim_mask dilated by one row up and down, edge nodes excluded (compact node list)
+  const unsigned *dil2_bits;             // lim_mask dilated by two rows up and down (all nodes)
   const double *lim_r, *lim_z;    // [nlim]
+  const int *lim_n0;              // [nlim] flat index of the lower-left node of each vertex's bilinear cell
+  const double *lim_tx, *lim_ty;  // [nlim] bilinear weights inside that cell
   // Delta* solve factors: [nri][nzi] (i-major so that threads over m coalesce)
   const double *tri_w, *tri_invb; // Thomas multipliers and inverse pivots
   const double *tri_ce;           // [nri] super-diagonal

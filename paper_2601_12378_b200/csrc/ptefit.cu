@@ -210,9 +210,41 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
       for (int i = 0; i < D.nr; ++i)
         if (i == 0 || j == 0 || i == D.nr - 1 || j == D.nz - 1) { const size_t n = (size_t)j * D.nr + i; eb[n >> 5] |= 1u << (n & 31); }
     TRY(upload(h, &D.edge_bits, eb.data(), eb.size()));
+    std::vector<unsigned> db((N + 31) / 32, 0u);
+    for (int j = 1; j < D.nz - 1; ++j)
+      for (int i = 1; i < D.nr - 1; ++i) {
+        const size_t n = (size_t)j * D.nr + i;
+        if (ge->lim_mask[n] || ge->lim_mask[n + D.nr] || ge->lim_mask[n - D.nr]) db[n >> 5] |= 1u << (n & 31);
+      }
+    TRY(upload(h, &D.dil_bits, db.data(), db.size()));
+    std::vector<unsigned> d2((N + 31) / 32, 0u);
+    for (int j = 0; j < D.nz; ++j)
+      for (int i = 0; i < D.nr; ++i) {
+        bool any = false;
+        for (int dj = -2; dj <= 2; ++dj)
+          if (j + dj >= 0 && j + dj < D.nz && ge->lim_mask[(size_t)(j + dj) * D.nr + i]) any = true;
+        const size_t n = (size_t)j * D.nr + i;
+        if (any) d2[n >> 5] |= 1u << (n & 31);
+      }
+    TRY(upload(h, &D.dil2_bits, d2.data(), d2.size()));
   }
   TRY(upload(h, &D.lim_r, ge->lim_r, (size_t)D.nlim));
   TRY(upload(h, &D.lim_z, ge->lim_z, (size_t)D.nlim));
+  {
+    // bilinear cell and weights of every limiter vertex (same FP64 expressions as search_body)
+    std::vector<int> n0(D.nlim);
+    std::vector<double> tx(D.nlim), ty(D.nlim);
+    for (int v = 0; v < D.nlim; ++v) {
+      const double fi = (ge->lim_r[v] - D.rmin) / D.dr, fj = (ge->lim_z[v] - D.zmin) / D.dz;
+      int i0 = (int)floor(fi), j0 = (int)floor(fj);
+      i0 = i0 < 0 ? 0 : (i0 > D.nr - 2 ? D.nr - 2 : i0);
+      j0 = j0 < 0 ? 0 : (j0 > D.nz - 2 ? D.nz - 2 : j0);
+      n0[v] = j0 * D.nr + i0; tx[v] = fi - i0; ty[v] = fj - j0;
+    }
+    TRY(upload(h, &D.lim_n0, n0.data(), n0.size()));
+    TRY(upload(h, &D.lim_tx, tx.data(), tx.size()));
+    TRY(upload(h, &D.lim_ty, ty.data(), ty.size()));
+  }
   // Delta* factors ("the coefficient matrices can be pre-computed"): for each DST
   // mode m the tridiagonal [cw_i, -2/dR^2 + lam_m, ce_i] is LU-factored in FP64 on the host.
   {

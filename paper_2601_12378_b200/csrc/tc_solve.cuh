@@ -23,6 +23,7 @@
 #include "common.cuh"
 #include "search_kernels.cuh"
 #include "fused_solve.cuh"
+#include "search_lean.cuh"
 #include "tc_gemm.cuh"
 
 namespace ptefit {
@@ -46,7 +47,7 @@ struct TcSolveDev {
 __host__ __device__ inline size_t tcs_smem_bytes(int nr, int nz) {
   const size_t N = (size_t)nr * nz, nwords = (N + 31) / 32;
   size_t b = 1024 + TCS_TAB_BYTES + TCS_OP_BYTES;          // alignment slack + tables + operands (flux map aliases the operands)
-  b += 3 * nwords * sizeof(unsigned);                      // lim / xpt / edge bit masks
+  b += 4 * nwords * sizeof(unsigned);                      // lim / xpt / dilated lim (1 and 2 rows) bit masks
   b += (size_t)(2 * (nr + nz)) * sizeof(float);            // boundary flux
   b += 2 * (size_t)nr * sizeof(double);                    // sub- and super-diagonal
   return b + 64;
@@ -68,10 +69,12 @@ __device__ __forceinline__ void tmem_ld16u(uint32_t taddr, uint32_t *r) {
       : "r"(taddr));
   asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
 }
-__device__ __forceinline__ uint32_t tf32_bits(float v) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(r) : "f"(v));
-  return r;
+// a = hi + lo for the 3xTF32 products: hi = a rounded to TF32 (nearest, ties away: add half an ulp of the
+// 10-bit mantissa, clear the low 13 bits -- cvt.rna.tf32.f32 costs four instructions on sm_100a, this
+// two), lo = a - hi exactly; the tensor core ignores the low 13 bits of lo itself.
+__device__ __forceinline__ void tf32_split(float v, uint32_t &hi, uint32_t &lo) {
+  hi = (__float_as_uint(v) + 0x1000u) & 0xffffe000u;
+  lo = __float_as_uint(v - __uint_as_float(hi));
 }
 
 // Byte offset of element (row n, k) inside a [128 rows][64 k] FP32 operand stored as two K-blocks of
@@ -108,15 +111,16 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   using T = float;
   extern __shared__ unsigned char smem_dyn[];
   if (!psi_all) psi_all = reinterpret_cast<T *>(D.ca->psi);
-  unsigned char *base = reinterpret_cast<unsigned char *>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+  unsigned char *base = smem_dyn + ((1024u - (tc::smem_u32(smem_dyn) & 1023u)) & 1023u);   // pointer arithmetic only: keeps the shared address space
   unsigned char *tab = base;                               // [hi kb0][hi kb1][lo kb0][lo kb1], 16 KB each
   unsigned char *op = base + TCS_TAB_BYTES;                // forward: E+ hi, E+ lo, E- hi, E- lo; inverse: Xo hi, Xo lo, Xe hi, Xe lo
-  T *G = reinterpret_cast<T *>(op);                        // flux map, aliases the operand tiles once they are consumed
+  T *Gb = reinterpret_cast<T *>(op);                       // flux map, aliases the operand tiles once they are consumed
+  const bool vec_ok = ((reinterpret_cast<uintptr_t>(psi_all) | reinterpret_cast<uintptr_t>(D.psi_coil)) & 15) == 0;
   const int nr = D.nr, nz = D.nz, N = D.N, nri = D.nri, nzi = D.nzi, Nz = nz - 1;
   const int nwords = (N + 31) >> 5;
-  unsigned *mbits = reinterpret_cast<unsigned *>(op + TCS_OP_BYTES);   // lim, xpt, edge bit masks
-  T *pb = reinterpret_cast<T *>(mbits + 3 * nwords);       // bottom[nr], top[nr], left[nzi], right[nzi]
-  double *ce_s = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(pb + 2 * (nr + nz)) + 7) & ~(uintptr_t)7);
+  unsigned *mbits = reinterpret_cast<unsigned *>(op + TCS_OP_BYTES);   // lim, xpt, dilated-lim bit masks
+  T *pb = reinterpret_cast<T *>(mbits + 4 * nwords);       // bottom[nr], top[nr], left[nzi], right[nzi]
+  double *ce_s = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(pb + 2 * (nr + nz)) + ((8u - (tc::smem_u32(pb + 2 * (nr + nz)) & 7u)) & 7u));
   double *cw_s = ce_s + nr;
   const double *ibs = reinterpret_cast<const double *>(op);   // Thomas phase: inverse pivots [i][lane], staged by bulk copies
   __shared__ uint64_t bar_tab, bar_mma, bar_ib[8];
@@ -124,6 +128,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
   __shared__ T pcoef[2 * (PTEFIT_MAX_DEG + 1)];
   __shared__ T c_edge[2];
+  __shared__ LeanShared lean;
   const int tid = threadIdx.x, nth = blockDim.x, warp = tid >> 5, lane = tid & 31;
   const bool elected = (tid == 4 * 32);                    // lane 0 of warp 4: TMA + MMA issue (warps 0-3 run the Thomas sweeps)
 
@@ -135,8 +140,8 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
     tc::fence_barrier_init();
   }
   if (warp == 0) tc::tmem_alloc<512>(&tmem_slot);
-  for (int w = tid; w < 3 * nwords; w += nth)
-    mbits[w] = (w < nwords) ? D.lim_bits[w] : (w < 2 * nwords) ? D.xpt_bits[w - nwords] : D.edge_bits[w - 2 * nwords];
+  for (int w = tid; w < 4 * nwords; w += nth)
+    mbits[w] = (w < nwords) ? D.lim_bits[w] : (w < 2 * nwords) ? D.xpt_bits[w - nwords] : (w < 3 * nwords) ? D.dil_bits[w - 2 * nwords] : D.dil2_bits[w - 3 * nwords];
   for (int i = tid; i < nr; i += nth) {
     const double Rd = D.rmin + i * D.dr;
     c_rhs[i] = T(-kMu0 * Rd / D.dA);
@@ -169,6 +174,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   constexpr uint32_t idesc128 = tc::idesc_tf32(128, 128), idesc64 = tc::idesc_tf32(128, 64);
 
 #ifdef PTEFIT_TUNING
+  if (tid == 0) for (int k = 0; k < 8; ++k) lean.clk[k] = 0;
   long long tcs_clk[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tcs_t0 = clock64();
 #endif
   for (int s = blockIdx.x; s < B; s += gridDim.x) {
@@ -176,6 +182,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
     const T *pbg = pbd_all + (size_t)s * D.nbnd;
     T *psi = psi_all + (size_t)s * N;
     const T *pc = D.psi_coil + (size_t)s * N;
+    T *G = Gb + (vec_ok ? (int)(((size_t)s * N) & 3) : 0);     // G + n is 16-byte aligned exactly when psi + n is
     __syncthreads();                                       // previous slice done with G and pb
     for (int k = tid; k < D.nbnd; k += nth) pb[k] = pbg[k];
     if (do_search && D.has_delz && tid < 2 * (PTEFIT_MAX_DEG + 1)) {
@@ -227,8 +234,8 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
           if (!valid) { a = 0.f; b = 0.f; }
           if (jj >= 63) b = 0.f;                            // mid row has no partner
           const float ep = a + b, em = a - b;
-          ph[t] = tf32_bits(ep); pl[t] = tf32_bits(ep - __uint_as_float(ph[t]));
-          mh[t] = tf32_bits(em); ml[t] = tf32_bits(em - __uint_as_float(mh[t]));
+          tf32_split(ep, ph[t], pl[t]);
+          tf32_split(em, mh[t], ml[t]);
         }
         const uint32_t off = tcs_off(n, 4 * q);
         *reinterpret_cast<uint4 *>(op + off) = make_uint4(ph[0], ph[1], ph[2], ph[3]);
@@ -291,18 +298,15 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
 #pragma unroll
         for (int u = 15; u >= 0; --u) {
           const int i = i0 + u;
-          float xh = 0.f, xl = 0.f;
+          float xf = 0.f;
           if (i < nri) {
             const double zz = __hiloint2double((int)zhi[u], (int)zlo[u]);
             x = fma(-(ce_s[i] * ibs[i * 128 + L]), x, zz);
-            xh = __uint_as_float(tf32_bits((float)x));
-            xl = __uint_as_float(tf32_bits((float)(x - (double)xh)));
+            xf = (float)x;
           }
-          zlo[u] = __float_as_uint(xh);
-          zhi[u] = __float_as_uint(xl);
+          zlo[u] = __float_as_uint(xf);
         }
-        tmem_st16(ya + i0, zlo);                           // x_hi over z's low words, x_lo over its high words
-        tmem_st16(ya + 128 + i0, zhi);
+        tmem_st16(ya + i0, zlo);                           // x (FP32) over z's low words; split hi / lo by all warps below
       }
       tmem_wait_st();
       tc::tc_fence_before();
@@ -331,14 +335,16 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
 #pragma unroll
       for (int hf = 0; hf < 2; ++hf) {
         const int i0 = 32 * g + 16 * hf;
-        uint32_t xh[16], xl[16];
-        tmem_ld16u(tl + i0, xh);
-        tmem_ld16u(tl + 128 + i0, xl);
+        uint32_t xv[16];
+        tmem_ld16u(tl + i0, xv);
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
           const uint32_t off = tcs_off(i0 + u, kx);
-          *reinterpret_cast<uint32_t *>(xt + off) = xh[u];
-          *reinterpret_cast<uint32_t *>(xt + 32768 + off) = xl[u];
+          const float xf = __uint_as_float(xv[u]);
+          uint32_t xh, xl;
+          tf32_split(xf, xh, xl);
+          *reinterpret_cast<uint32_t *>(xt + off) = xh;
+          *reinterpret_cast<uint32_t *>(xt + 32768 + off) = xl;
         }
       }
       tc::fence_proxy_async();
@@ -388,61 +394,78 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
     tc::tc_fence_before();
     __syncthreads();
     TCS_T(3);
-    // ---- total flux + relaxation; psi goes to global memory and stays in G for the search
-    SearchOpt<T> so_opt;
-    so_opt.am.v = -INFINITY; so_opt.am.n = 0x7fffffff;
+    // ---- total flux + relaxation; psi goes to global memory and stays in G for the search.  Flat over the
+    // nodes in 16-byte vectors (G is offset inside its buffer so that G + n and psi + n are aligned together);
+    // pass 0 of the search (finiteness, arg-max of s psi over lim_mask) rides along.
+    float am_v = -INFINITY;
+    int am_n = 0x7fffffff;
+    bool bad0 = false;
     {
-      constexpr int EB = 8;
-      const T sgT = T(D.ip_sign);
-      T am_v = -INFINITY;
-      int am_n = 0x7fffffff;
-      for (int n0 = tid; n0 < N; n0 += EB * nth) {
-        T cv[EB], ov[EB];
+      const float sgT = float(D.ip_sign);
+      float chk = 0.f;                                      // stays 0 unless a flux value is Inf / NaN
+      const int a0 = vec_ok ? min(N, (4 - (int)(((size_t)s * N) & 3)) & 3) : N;      // scalar head up to the first aligned node
+      const int nq = (N - a0) >> 2, t0 = a0 + 4 * nq;
+      // 16-byte body first (strict > keeps the smallest n of equal keys: a thread sees its nodes in increasing n)
+      constexpr int EB = 3;
+      for (int q0 = tid; q0 < nq; q0 += EB * nth) {
+        float4 cv[EB], ov[EB];
 #pragma unroll
         for (int u = 0; u < EB; ++u) {
-          const int n = n0 + u * nth;
-          cv[u] = (add_coil && n < N) ? pc[n] : T(0);
-          ov[u] = (use_relax && n < N) ? psi[n] : T(0);
+          const int q = q0 + u * nth;
+          cv[u] = (add_coil && q < nq) ? *reinterpret_cast<const float4 *>(pc + a0 + 4 * q) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ov[u] = (use_relax && q < nq) ? *reinterpret_cast<const float4 *>(psi + a0 + 4 * q) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int u = 0; u < EB; ++u) {
-          const int n = n0 + u * nth;
-          if (n < N) {
-            const unsigned bit = 1u << (n & 31);
-            T v = G[n] + cv[u];
-            if (use_relax) v = ov[u] + om * (v - ov[u]);
-            psi[n] = v;
-            G[n] = v;
-            if (do_search) {
-              so_opt.bad |= !isfinite(v);
-              const T key = sgT * v;
-              if ((mbits[n >> 5] & bit) && (key > am_v || (key == am_v && n < am_n))) { am_v = key; am_n = n; }
+          const int q = q0 + u * nth, n = a0 + 4 * q;
+          if (q < nq) {
+            const float4 g = *reinterpret_cast<const float4 *>(G + n);
+            const unsigned lb = __funnelshift_r(mbits[n >> 5], mbits[(n >> 5) + 1], n & 31);   // lim bits of nodes n..n+3
+            float v[4] = {g.x + cv[u].x, g.y + cv[u].y, g.z + cv[u].z, g.w + cv[u].w};
+            const float o[4] = {ov[u].x, ov[u].y, ov[u].z, ov[u].w};
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+              if (use_relax) v[t] = fmaf(om, v[t] - o[t], o[t]);
+              chk = fmaf(v[t], 0.f, chk);
+              const float key = sgT * v[t];
+              if (((lb >> t) & 1u) && key > am_v) { am_v = key; am_n = n + t; }
             }
+            const float4 r = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4 *>(psi + n) = r;
+            *reinterpret_cast<float4 *>(G + n) = r;
           }
         }
       }
-      so_opt.am.v = (double)am_v;
-      so_opt.am.n = am_n;
+      for (int n = tid; n < a0 + (N - t0); n += nth) {     // unaligned head and tail nodes
+        const int m = n < a0 ? n : t0 + (n - a0);
+        float v = G[m] + (add_coil ? pc[m] : 0.f);
+        if (use_relax) { const float o = psi[m]; v = fmaf(om, v - o, o); }
+        psi[m] = v; G[m] = v;
+        chk = fmaf(v, 0.f, chk);
+        const float key = sgT * v;
+        if (((mbits[m >> 5] >> (m & 31)) & 1u) && (key > am_v || (key == am_v && m < am_n))) { am_v = key; am_n = m; }
+      }
+      bad0 = !(chk == 0.f);
     }
     __syncthreads();
     TCS_T(4);
     if (do_search) {
-      T *xn = xn_all + (size_t)s * N;
-      so_opt.lbits = mbits; so_opt.xbits = mbits + nwords; so_opt.have_am = true;
-      so_opt.local = G;
-      if (D.has_delz) { so_opt.pc = pcoef; so_opt.rdA = c_rdA; so_opt.fdA = c_fdA; so_opt.Xs = D.X + (size_t)s * D.nt; }
-      search_body<T>(D, s, G, xn, so_opt);                 // G now holds I'(xn) (delz) or xn
+      float *xn = xn_all + (size_t)s * N;
+      search_lean(D, lean, s, G, xn, mbits, mbits + nwords, mbits + 3 * nwords, am_v, am_n, bad0, D.has_delz ? pcoef : nullptr, c_rdA, c_fdA,
+                  D.X + (size_t)s * D.nt);                 // G now holds I'(xn) (delz) or xn on the lim_mask words
       TCS_T(5);
       if (D.has_delz) {
+        // -dI'/dZ column for the NEXT fit, on the nodes of the compact list only (lim_mask dilated by one row;
+        // everything else keeps the zero of the memset at the start of the call)
         __syncthreads();
-        T *dzc = D.dzc + (size_t)s * N;
-        const T hz = T(0.5 / D.dz);
-        const unsigned *ebits = mbits + 2 * nwords;
-#pragma unroll 4
-        for (int n = tid; n < N; n += nth) {
-          const bool edge = (ebits[n >> 5] >> (n & 31)) & 1u;
-          const int up = edge ? n : n + nr, dn = edge ? n : n - nr;
-          dzc[n] = edge ? T(0) : -(G[up] - G[dn]) * hz;
+        float *dzc = D.dzc + (size_t)s * N;
+        const float hz = float(0.5 / D.dz);
+        const unsigned *dbits = mbits + 2 * nwords;
+        for (int w = warp; w < nwords; w += nth >> 5) {
+          const unsigned dw = dbits[w];
+          if (!dw) continue;
+          const int n = (w << 5) + lane;
+          if ((dw >> lane) & 1u) dzc[n] = -(G[n + nr] - G[n - nr]) * hz;     // G = 0 off the lim_mask nodes (search_lean)
         }
       }
       TCS_T(6);
@@ -452,6 +475,9 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   if (tid == 0 && blockIdx.x == 0 && do_search)
     printf("k_solve_tc cycles: rhs %lld fwd+thomas %lld inv %lld unfold %lld total-flux %lld search %lld delz %lld | mma-wait %lld fwd-sweep %lld bwd-sweep %lld (tmem-ld %lld ib-wait %lld)\n", tcs_clk[0], tcs_clk[1],
            tcs_clk[2], tcs_clk[3], tcs_clk[4], tcs_clk[5], tcs_clk[6], tcs_clk[7], tcs_clk[8], tcs_clk[9], tcs_clk[10], tcs_clk[11]);
+  if (tid == 0 && blockIdx.x == 0 && do_search)
+    printf("  search_lean cycles: argmax+axis %lld scan %lld decide %lld limiter %lld pb %lld mask %lld tail %lld nlist %d ncand %d\n", lean.clk[0], lean.clk[1], lean.clk[2],
+           lean.clk[3], lean.clk[4], lean.clk[5], lean.clk[6], lean.nlist, lean.ncand);
 #endif
   tc::tc_fence_before();
   __syncthreads();
