@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libptefit.so")
 SOURCES = ["ptefit.cu"]
-DEPS = ["common.cuh", "fit_kernels.cuh", "search_kernels.cuh", "solve_kernels.cuh", "fused_solve.cuh", "tc_gemm.cuh", "tc_kernels.cuh", "tc_solve.cuh", "tc_host.inc", "launch.inc", "ptefit.cu",
+DEPS = ["common.cuh", "fit_kernels.cuh", "search_kernels.cuh", "solve_kernels.cuh", "fused_solve.cuh", "tc_gemm.cuh", "tc_kernels.cuh", "tc_solve.cuh", "search_lean.cuh", "dmma_gemm.cuh", "dmma_kernels.cuh", "dm_host.inc", "tc_host.inc", "launch.inc", "ptefit.cu",
         os.path.join("..", "..", "include", "ptefit.h")]
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]

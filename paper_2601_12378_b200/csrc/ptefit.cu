@@ -19,6 +19,8 @@
 #include "tc_gemm.cuh"
 #include "tc_kernels.cuh"
 #include "tc_solve.cuh"
+#include "dmma_gemm.cuh"
+#include "dmma_kernels.cuh"
 
 using namespace ptefit;
 
@@ -41,6 +43,8 @@ struct ptefit_handle {
   const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;
   int pbd_ntiles = 0, max_split_resp = 1, max_split_pbd = 1;
   const float *c_rdA = nullptr, *c_fdA = nullptr;   // Eq. 10 factors on the compact node list
+  bool dm = false;                      // FP64 tensor-core (DMMA) contractions usable (FP64 mode, gemm != FFMA)
+  DmDev Dm{};
   bool tcs = false;                     // k_solve_tc usable (FP32, N_Z = 129, tensor-core mode)
   TcSolveDev Ts{};
   size_t tcs_smem = 0;
@@ -334,6 +338,7 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
 }
 
 #include "tc_host.inc"
+#include "dm_host.inc"
 
 extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geometry *ge,
                                        const ptefit_tables *tb, const ptefit_basis *ba,
@@ -413,6 +418,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   ptefit_status st = (h->prec == PTEFIT_FP32) ? build(h, h->d32, g, ge, tb, ba, op->max_batch)
                                               : build(h, h->d64, g, ge, tb, ba, op->max_batch);
   if (st == PTEFIT_OK && h->prec == PTEFIT_FP32 && h->gemm != PTEFIT_GEMM_FFMA) { st = build_tc(h, h->d32, ge, tb, op->max_batch); if (st == PTEFIT_OK) st = build_tcsolve(h, h->d32); }
+  if (st == PTEFIT_OK && h->prec == PTEFIT_FP64 && h->gemm != PTEFIT_GEMM_FFMA) st = build_dm(h, h->d64, ge, tb, op->max_batch);
   if (st != PTEFIT_OK) { std::string e = h->error; ptefit_destroy(h); g_error = e; return st; }
   *out = h;
   return PTEFIT_OK;

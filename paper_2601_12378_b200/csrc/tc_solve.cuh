@@ -332,9 +332,10 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
       const int q = warp & 3, g = warp >> 2, L = q * 32 + lane, kx = L & 63;
       const uint32_t tl = tmem_base + ((uint32_t)(q * 32) << 16) + 256u;
       unsigned char *xt = op + (L < 64 ? 0 : 65536);
+      constexpr int CPG = 128 / (TCS_THREADS / 128);         // columns per group of four warps
 #pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
-        const int i0 = 32 * g + 16 * hf;
+      for (int hf = 0; hf < CPG / 16; ++hf) {
+        const int i0 = CPG * g + 16 * hf;
         uint32_t xv[16];
         tmem_ld16u(tl + i0, xv);
 #pragma unroll
@@ -371,9 +372,11 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
       const int q = warp & 3, g = warp >> 2, n = q * 32 + lane, gi = n + 1;
       const uint32_t tl = tmem_base + ((uint32_t)(q * 32) << 16);
       uint32_t a[16], b[16];
-      tmem_ld16u(tl + 16 * g, a);
-      tmem_ld16u(tl + 64 + 16 * g, b);
-      if (n < nri) {
+      if (g < 4) {
+        tmem_ld16u(tl + 16 * g, a);
+        tmem_ld16u(tl + 64 + 16 * g, b);
+      }
+      if (g < 4 && n < nri) {
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
           const int jj = 16 * g + t, j = jj + 1;
