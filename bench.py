@@ -85,6 +85,35 @@ class ClockSampler:
                     reasons=sorted(reasons), samples=len(sm))
 
 
+def yardsticks(torch):
+    """Library GEMMs timed on this box in this run (yardsticks only): TF32 and FP64
+    torch.matmul, best of 5 after warm-up.  TFLOP/s."""
+    out = {}
+    prev = torch.backends.cuda.matmul.allow_tf32
+    for name, dt, n, tf32 in (("tf32_tflops", torch.float32, 8192, True), ("fp64_tflops", torch.float64, 4096, False)):
+        torch.backends.cuda.matmul.allow_tf32 = tf32
+        a = torch.randn(n, n, dtype=dt, device="cuda"); b = torch.randn(n, n, dtype=dt, device="cuda")
+        for _ in range(2):
+            a @ b
+        best = 1e30
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); a @ b; e1.record(); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        out[name] = 2.0 * n ** 3 / (best * 1e-3) / 1e12
+        del a, b
+    torch.backends.cuda.matmul.allow_tf32 = prev
+    out["how"] = "torch.matmul 8192^3 with TF32 allowed / 4096^3 FP64, best of 5, CUDA events (library yardsticks)"
+    return out
+
+
+def ncu_traffic():
+    """DRAM bytes per launch of the stage kernels from the committed `ncu --set full` summaries
+    (profiles/r2_ncu_traffic.json: dram__bytes_read.sum + dram__bytes_write.sum, workload cfg4 batch 512)."""
+    p = os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
 def make_workload(name, batch, first=0):
     """Seeded synthetic device + `batch` slices (synth/)."""
     import synth
@@ -162,20 +191,28 @@ def stage_roofline(stage, ms_per_launch, dims, peaks, gemm_mode):
     Algorithmic work per launch = SURVEY.md 8(d)'s per-slice figure x slices per launch."""
     B, es = dims["B"], dims["es"]
     N, Nint, Nb, M, nt = dims["N"], dims["Nint"], dims["Nb"], dims["M"], dims["nt"]
-    tf32 = 0.5 * peaks["bf16_sustained"]           # guide: nominal TF32 dense = 1/2 of bf16 dense
+    tf32 = peaks.get("tf32") or (1.1 / 2.25) * peaks["bf16_sustained"]   # measured yardstick, else the guide's nominal TF32 : bf16 ratio
+    tnote = peaks.get("tf32_note", "1.1/2.25 x measured sustained bf16")
+    fp64 = peaks.get("fp64") or 37.0
+    f64 = es == 8
     if stage == "response":
         flops = 2.0 * M * Nint * nt * B
-        return dict(kernel="k_basis_split+k_gemm_3xtf32<144,3>+k_resp_reduce", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
-                    unit="TFLOP/s", peak_note=f"0.5 x measured sustained bf16 ({peaks['source']}); gemm mode {gemm_mode}")
+        return dict(kernel="k_basis_c+k_gemm_dmma+k_resp_reduce_d" if f64 else "k_gemm_3xtf32<144,3,NP,NFF>+k_resp_reduce", bound="tensor",
+                    achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=fp64 if f64 else tf32, unit="TFLOP/s",
+                    peak_note=("FP64 yardstick" if f64 else tnote) + f"; gemm mode {gemm_mode}; algorithmic flops on the full node list (2 M N_int nb)")
     if stage == "boundary":
         flops = 2.0 * Nb * Nint * B
-        return dict(kernel="k_cur_split+k_gemm_3xtf32<256,2>+k_pbd_reduce", bound="tensor", achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=tf32,
-                    unit="TFLOP/s", peak_note=f"0.5 x measured sustained bf16 ({peaks['source']}); gemm mode {gemm_mode}")
+        return dict(kernel="k_current_c+k_gemm_dmma+k_pbd_reduce_d" if f64 else "k_current_split+k_gemm_3xtf32<256,2>+k_pbd_reduce", bound="tensor",
+                    achieved=flops / (ms_per_launch * 1e-3) / 1e12, peak=fp64 if f64 else tf32, unit="TFLOP/s",
+                    peak_note=("FP64 yardstick" if f64 else tnote) + f"; gemm mode {gemm_mode}")
     if stage == "solve" and dims.get("fused"):
-        # k_solve_fused: read I, psi_coil, old psi; write psi, normalised flux, delz column (+ boundary flux)
-        byts = float(es) * (6 * N + Nb) * B
-        return dict(kernel="k_solve_fused", bound="hbm", achieved=byts / (ms_per_launch * 1e-3) / 1e9,
-                    peak=peaks["hbm"], unit="GB/s", peak_note=f"{peaks['source']} copy bandwidth")
+        # SURVEY.md 8(d): A7 + A8 read 4 N_int (J) + 4 N (psi_coil), write 4 N (psi); A1 fused behind it writes <= 5 N
+        byts = (float(es) * (Nint + 2 * N) + (es + 1.0) * N) * B
+        # what the kernel moves with this repo's additions: + old psi (relaxation), + delz column, + boundary flux
+        extra = float(es) * (6 * N + Nb) * B
+        return dict(kernel="k_solve_tc" if not f64 and dims.get("tcs") else "k_solve_fused", bound="hbm", achieved=byts / (ms_per_launch * 1e-3) / 1e9,
+                    peak=peaks["hbm"], unit="GB/s", peak_note=f"{peaks['source']} copy bandwidth; algorithmic bytes per SURVEY.md 8(d)",
+                    bytes_per_launch=byts, bytes_incl_additions=extra)
     if stage == "solve":
         byts = float(es) * (Nint + N + N + N) * B    # read I, psi_coil, old psi (relaxation); write psi
         return dict(kernel="k_rhs_dst+k_tridiag+k_idst_total", bound="hbm", achieved=byts / (ms_per_launch * 1e-3) / 1e9,
@@ -208,7 +245,7 @@ def run_ours(args):
     prec = c["precision"]
     n_iter = c["n_iter"]
     # each rank reconstructs its own B slices (weak scaling: slices are independent, tables replicated)
-    n_unique = min(B, args.unique)
+    n_unique = min(B, args.unique) if args.unique > 0 else B
     dev, sl = make_workload(args.config, n_unique, first=rank * n_unique)
     reps = (B + n_unique - 1) // n_unique
     b_np = np.tile(sl["b"], (reps, 1))[:B]
@@ -268,20 +305,25 @@ def run_ours(args):
     dims["fused"] = "search" not in loop_stages     # search runs inside k_solve_fused
     top = max(loop_stages, key=loop_stages.get)
     peaks = _peaks()
+    yard = None
+    if not args.skip_extras:
+        yard = yardsticks(torch)
+        peaks["tf32"] = yard["tf32_tflops"]; peaks["fp64"] = yard["fp64_tflops"]
+        peaks["tf32_note"] = "TF32 torch.matmul yardstick measured in this run"
+    dims["tcs"] = (prec == "fp32" and rec.nz == 129 and rec.nr <= 129)
     roof = stage_roofline(top, loop_stages[top] / n_iter, dims, peaks, args.gemm)
     roof["frac"] = roof["achieved"] / roof["peak"]
-    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the committed
-    # `ncu --set full` capture of this workload, profiles/r1_final_ncu_full.md; null for other workloads
-    ncu_traffic = {"k_solve_fused": 216.7e6, "response": 54.1e6, "boundary": 65.8e6}
     roof["traffic"] = None
     if args.config == "cfg4" and B == 512:
-        roof["traffic"] = ncu_traffic.get("k_solve_fused" if top == "solve" else top)
+        roof["traffic"] = ncu_traffic().get(roof["kernel"].split("+")[0].split("<")[0])
     roof["share_of_step"] = loop_stages[top] / max(sum(acc.values()), 1e-9)
     roof["all_stages"] = {}
     for sname, ms in loop_stages.items():
         r = stage_roofline(sname, ms / n_iter, dims, peaks, args.gemm)
         roof["all_stages"][sname] = dict(ms_per_step=ms, bound=r["bound"], achieved=r["achieved"], unit=r["unit"],
                                          frac=r["achieved"] / r["peak"])
+        if r["bound"] == "tensor" and prec == "fp32":
+            roof["all_stages"][sname]["frac_of_peak_over_3"] = 3.0 * r["achieved"] / r["peak"]     # 3xTF32 issues three MMAs per product
     e2e = None
     if not args.skip_extras:
         e2e = run_e2e(args, torch, dist, rec, b_np, ic_np, dt, B, n_iter, world, barrier)
@@ -295,12 +337,12 @@ def run_ours(args):
                            l2="flushed between timed steps (256 MB memset) and working set > L2",
                            parallelism=f"slices sharded over {world} GPU(s), no collective"),
                clocks=clocks, e2e=e2e, gpu_launches=launches, slices_status_ok=n_ok, roofline=roof,
-               stage_ms_per_step=acc)
+               stage_ms_per_step=acc, yardsticks=yard)
     if rank == 0 and world == 1 and not args.skip_extras:
         out["latency_batch1"] = latency_batch1(args, torch, P)
         dv, b32, ic32 = round32(dev, sl) if prec == "fp32" else (dev, sl["b"], sl["ic"])
         v, done, secs = oracle_throughput(dv, b32, ic32, n_iter, args.cpu_sample)
-        out["cpu_baseline"] = dict(value=v, unit=UNIT, cores=host_threads(), kind="oracle",
+        out["cpu_baseline"] = dict(value=v, unit=UNIT, cores=host_threads(), kind="oracle", note="the numpy test oracle as it stands, not a tuned CPU baseline",
                                    sample=f"first {done} slices of the same {args.config} batch, {n_iter} iterations each, {secs:.1f} s")
     if rank == 0:
         print(json.dumps(out), flush=True)
@@ -364,8 +406,26 @@ def latency_batch1(args, torch, P):
         e0.record(); rec.reconstruct(d_b, d_ic, 1, warm_start=True); e1.record()
         torch.cuda.synchronize()
         tw.append(e0.elapsed_time(e1))
+    # streaming replay (PAPER.md:158, 175 / Fig. 3): 10 000 consecutive slices, one warm-started Picard
+    # iteration each (the previous slice's flux is the start), measurements cycling through the stored
+    # cfg3 slices; one event pair per slice, read after the loop
+    dev8, sl8 = make_workload("cfg3", 8)
+    d_b8 = torch.tensor(sl8["b"], dtype=rec.dtype, device="cuda")
+    d_ic8 = torch.tensor(sl8["ic"], dtype=rec.dtype, device="cuda")
+    n_stream = 10000
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(n_stream + 1)]
+    evs[0].record()
+    for q in range(n_stream):
+        k = (q // 250) % 8                                   # the equilibrium changes every 250 slices
+        rec.reconstruct(d_b8[k:k + 1], d_ic8[k:k + 1], 1, warm_start=True)
+        evs[q + 1].record()
+    torch.cuda.synchronize()
+    st = np.array([evs[q].elapsed_time(evs[q + 1]) for q in range(n_stream)]) * 1e3
+    stream = dict(slices=n_stream, us_mean=float(st.mean()), us_p50=float(np.percentile(st, 50)), us_p99=float(np.percentile(st, 99)),
+                  us_max=float(st.max()), status_ok=int(rec.status[0].item() == 0),
+                  note="one warm-started Picard iteration per slice, back-to-back launches, no post-processing")
     rec.close()
-    return dict(workload="cfg3", us_per_slice=1e3 * float(np.median(ts)), us_min=1e3 * float(min(ts)), n_iter=c["n_iter"],
+    return dict(workload="cfg3", streaming=stream, us_per_slice=1e3 * float(np.median(ts)), us_min=1e3 * float(min(ts)), n_iter=c["n_iter"],
                 us_per_iteration=1e3 * float(np.median(ts)) / c["n_iter"],
                 us_one_warm_iteration=1e3 * float(np.median(tw)),
                 launches_per_call=n, paper_context="0.268 ms/slice at 129x129 on the paper's GPU (PAPER.md:175), other hardware")
@@ -379,7 +439,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--batch", type=int, default=0, help="override the config's batch")
-    ap.add_argument("--unique", type=int, default=128, help="distinct seeded slices per rank (tiled to the batch)")
+    ap.add_argument("--unique", type=int, default=0, help="distinct seeded slices per rank, tiled to the batch (0 = all distinct)")
     ap.add_argument("--gemm", default="3xtf32", help="contraction arithmetic label recorded in config")
     ap.add_argument("--cpu-sample", type=int, default=24, help="slices the cpu_baseline leg times")
     ap.add_argument("--skip-extras", action="store_true", help="timed region + stage breakdown only (for ncu runs)")

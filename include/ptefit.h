@@ -170,6 +170,18 @@ int ptefit_last_launch_count(const ptefit_handle *h);
 ptefit_status ptefit_set_profiling(ptefit_handle *h, int on);
 ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
 
+/* NEXT-3: a Green's table on the GPU (Sec. II.A, Eq. 3-5; closed forms
+ * with complete elliptic integrals, reading O1 of DESIGN.md).  out[k][c] = w_c g(field point k, source c)
+ * per ampere in the source filament: g = flux per radian psi (Eq. 5) for a flux row (d_fld_cos == NULL,
+ * or cos = sin = 0 for that row), g = cos a B_R + sin a B_Z for a probe row (Eq. 3-4).  All pointers are
+ * DEVICE memory, FP64; d_src_w may be NULL (weights 1: e.g. turn counts); transpose = 1 stores out[c][k].
+ * Coincident points give 0 (self terms are never needed: DESIGN.md O1).  Asynchronous on cuda_stream.
+ * No handle: the tables are inputs of ptefit_create. */
+ptefit_status ptefit_greens_table(int n_fld, const double *d_fld_r, const double *d_fld_z,
+                                  const double *d_fld_cos, const double *d_fld_sin,
+                                  int n_src, const double *d_src_r, const double *d_src_z,
+                                  const double *d_src_w, double *d_out, int transpose, void *cuda_stream);
+
 void ptefit_destroy(ptefit_handle *h);
 const char *ptefit_last_error(const ptefit_handle *h);
 const char *ptefit_global_error(void);

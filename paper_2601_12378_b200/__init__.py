@@ -5,4 +5,4 @@ Argument marshalling only -- every step of the Picard iteration runs in the CUDA
 checked), but creating a handle without a B200 raises.
 """
 from .binding import (PtefitError, Reconstructor, load_library, poly_terms,  # noqa: F401
-                      ptefit_create, ptefit_destroy, ptefit_reconstruct, EXPORTED_SYMBOLS, shard_slices)
+                      ptefit_create, ptefit_destroy, ptefit_reconstruct, ptefit_greens_table, EXPORTED_SYMBOLS, shard_slices)

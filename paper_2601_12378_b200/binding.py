@@ -11,7 +11,7 @@ LIB_PATH = os.path.join(HERE, "libptefit.so")
 EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
-    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms",
+    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
@@ -90,6 +90,8 @@ def load_library():
         lib.ptefit_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.ptefit_get_stage_ms.restype = C.c_int
         lib.ptefit_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        lib.ptefit_greens_table.restype = C.c_int
+        lib.ptefit_greens_table.argtypes = ([C.c_int] + [C.c_void_p] * 4 + [C.c_int] + [C.c_void_p] * 4 + [C.c_int, C.c_void_p])
         _lib = lib
     return _lib
 
@@ -276,6 +278,18 @@ class Reconstructor:
             self.close()
         except Exception:
             pass
+
+
+def ptefit_greens_table(d_fld_r, d_fld_z, d_src_r, d_src_z, d_out, d_fld_cos=None, d_fld_sin=None, d_src_w=None, transpose=False,
+                        stream=None):
+    """FP64 torch CUDA tensors in; d_out [n_fld, n_src] (or [n_src, n_fld] if transpose) is filled asynchronously."""
+    import torch
+    lib = load_library()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    st = lib.ptefit_greens_table(int(d_fld_r.numel()), _dp(d_fld_r), _dp(d_fld_z), _dp(d_fld_cos), _dp(d_fld_sin), int(d_src_r.numel()),
+                                 _dp(d_src_r), _dp(d_src_z), _dp(d_src_w), _dp(d_out), int(bool(transpose)), C.c_void_p(s.cuda_stream))
+    if st != 0:
+        raise PtefitError(f"ptefit_greens_table failed ({st}): {lib.ptefit_global_error().decode()}")
 
 
 def shard_slices(n_slices, rank, world):

@@ -21,6 +21,7 @@
 #include "tc_solve.cuh"
 #include "dmma_gemm.cuh"
 #include "dmma_kernels.cuh"
+#include "greens_kernels.cuh"
 
 using namespace ptefit;
 
@@ -434,6 +435,20 @@ extern "C" void ptefit_destroy(ptefit_handle *h) {
   if (h->gstream) cudaStreamDestroy(h->gstream);
   if (h->hstream) cudaStreamDestroy(h->hstream);
   delete h;
+}
+
+extern "C" ptefit_status ptefit_greens_table(int n_fld, const double *fr, const double *fz, const double *fcos, const double *fsin,
+                                             int n_src, const double *sr, const double *sz, const double *sw, double *out,
+                                             int transpose, void *cuda_stream) {
+  ptefit_handle *h = nullptr;
+  if (n_fld < 1 || n_src < 1 || n_fld > 65535 || !fr || !fz || !sr || !sz || !out || (!fcos) != (!fsin))
+    return fail(h, PTEFIT_ERR_INVALID_ARG, "ptefit_greens_table: bad arguments (1 <= n_fld <= 65535, n_src >= 1, non-null points)");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(h, PTEFIT_ERR_CUDA, "no CUDA device (there is no CPU fallback)");
+  k_greens_table<<<dim3((n_src + 255) / 256, n_fld), 256, 0, (cudaStream_t)cuda_stream>>>(n_fld, fr, fz, fcos, fsin, n_src, sr, sz, sw, out,
+                                                                                        transpose ? 1 : 0);
+  CK(cudaGetLastError());
+  return PTEFIT_OK;
 }
 
 extern "C" const char *ptefit_last_error(const ptefit_handle *h) { return h ? h->error.c_str() : g_error.c_str(); }

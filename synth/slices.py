@@ -1,11 +1,15 @@
 """Seeded per-slice inputs: measurement vectors b and coil currents I_C.
 
-Recipe: an analytic D-shaped current distribution of total I_p
-(polynomial in a geometric flux label, the shape BASELINE.json's "Solov'ev-like scale"
-describes) plus PF-coil currents chosen by a small regularised least squares so that the
-target boundary is an iso-flux contour of plasma + coils (and grad psi = 0 at the target
-X-points).  No Grad-Shafranov solve, no search, no basis fit happens here.
+`make_slices` loads the case files synth/cases/<cfg>.npz that the oracle-side script
+oracle/design_cases.py wrote (converged Grad-Shafranov equilibria of the fitted current form,
+DESIGN.md "Input recipe").  `truth_slice` is the seeded draw that script starts from: an analytic
+D-shaped current distribution of total I_p (polynomial in a geometric flux label) plus PF-coil
+currents from a small regularised least squares making the target boundary an iso-flux contour.
+No Grad-Shafranov solve, no search, no basis fit happens in this module.
 """
+import functools
+import os
+
 import numpy as np
 from .device import CONFIGS, MU0, filament_psi, filament_b, sensor_response
 
@@ -94,37 +98,34 @@ def truth_slice(dev, k):
     u = np.linalg.lstsq(Areg, yreg, rcond=None)[0]
     i_pf = u * rng_ic
     ic = np.concatenate([i_pf, i_eddy])
-    return dict(I=I.ravel(), ic=ic, shape=sh, ca=ca * scale, cb=cb * scale, ip=ip,
-                design_resid=float(np.max(np.abs(A @ i_pf - y))))
+    return dict(I=I.ravel(), ic=ic, shape=sh, ca=ca * scale, cb=cb * scale, ip=ip, ctl_r=cr, ctl_z=cz, i_eddy=i_eddy,
+                draw=draw, label=x, design_resid=float(np.max(np.abs(A @ i_pf - y))))
 
 
-def make_slices(dev, n_slices, first=0, noise=0.005, n_cal=None):
-    """b[n_slices, M], ic[n_slices, n_coil] (float64) for slices first..first+n_slices-1 and
-    sigma[M]: 0.5 % of the per-group (probes / loops) RMS of the noise-free signals over the
-    first n_cal slices (default min(config batch, 16)).  Fills dev['geom']['sigma'] if unset."""
-    meta, c, tb = dev["meta"], dev["meta"]["cfg"], dev["tables"]
-    npb = meta["n_probe"]
+CASE_DIR = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cases")
+
+
+@functools.lru_cache(maxsize=8)
+def _case_file(name):
+    path = os.path.join(CASE_DIR, name + ".npz")
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} is missing: run `python -m oracle.design_cases {name}` (the case files are written "
+                                "by the oracle-side design-Picard script; synth only loads them)")
+    with np.load(path) as f:
+        return {k: f[k] for k in f.files}
+
+
+def make_slices(dev, n_slices, first=0):
+    """b[n_slices, M], ic[n_slices, n_coil] (float64) for slices first..first+n_slices-1 of the config's
+    case file synth/cases/<cfg>.npz (indices wrap around the stored count) and sigma[M].  The file holds
+    converged Grad-Shafranov equilibria of the fitted current form + 0.5 % Gaussian noise, written by
+    oracle/design_cases.py.  Fills dev['geom']['sigma'] if unset.  `truth` carries what the generator
+    recorded per slice (coefficients, I_p, kind, designed axis / X-point)."""
+    cf = _case_file(dev["meta"]["name"])
+    n_store = cf["b"].shape[0]
+    idx = (first + np.arange(n_slices)) % n_store
     if dev["geom"]["sigma"] is None:
-        n_cal = n_cal or min(c["batch"], 16)
-        cal = np.stack([_clean(dev, k) for k in range(n_cal)])
-        sig = np.empty(cal.shape[1])
-        sig[:npb] = noise * np.sqrt(np.mean(cal[:, :npb] ** 2))
-        sig[npb:] = noise * np.sqrt(np.mean(cal[:, npb:] ** 2))
-        dev["geom"]["sigma"] = sig
-    sig = dev["geom"]["sigma"]
-    b = np.empty((n_slices, len(sig)))
-    ic = np.empty((n_slices, tb["gc"].shape[1]))
-    truth = []
-    for q in range(n_slices):
-        k = first + q
-        t = truth_slice(dev, k)
-        rng = np.random.default_rng((20260112 + c["idx"]) * 1000 + k + 500_000_000)
-        b[q] = tb["gp"] @ t["I"] + tb["gc"] @ t["ic"] + sig * rng.standard_normal(len(sig))
-        ic[q] = t["ic"]
-        truth.append(t)
-    return dict(b=b, ic=ic, sigma=sig, truth=truth)
-
-
-def _clean(dev, k):
-    t = truth_slice(dev, k)
-    return dev["tables"]["gp"] @ t["I"] + dev["tables"]["gc"] @ t["ic"]
+        dev["geom"]["sigma"] = cf["sigma"].copy()
+    truth = [dict(X=cf["X_true"][q], ip=float(cf["ip"][q]), kind=str(cf["kind"][q]), axis=cf["axis"][q], xpt=cf["xpt"][q],
+                  limited=int(cf["limited"][q]), seed=int(cf["seed"][q])) for q in idx]
+    return dict(b=cf["b"][idx].copy(), ic=cf["ic"][idx].copy(), sigma=cf["sigma"].copy(), truth=truth)
