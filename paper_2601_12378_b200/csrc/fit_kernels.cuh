@@ -246,6 +246,96 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
   }
 }
 
+// A4, second driver: modified Gram-Schmidt QR ("Gram-Schmidt QR ... stable, slower") of the
+// stacked, column-equilibrated, Tikhonov-augmented matrix [W R S^-1 ; lambda sqrt(M) I] in FP64, one warp
+// per slice, matrix in shared memory: (M + nt) rows x (nt + 1) columns (last column = right-hand side).
+// Same scaling, regularisation, chi^2 and status rules as k_lsq.  grid B, block 32,
+// dyn smem ((M + nt) (nt + 1) + nt (nt + 1) + nt) doubles.
+template <typename T>
+__global__ void __launch_bounds__(32) k_lsq_mgs(Dev<T> D, int B) {
+  extern __shared__ __align__(16) unsigned char mgs_raw[];
+  const int s = blockIdx.x, lane = threadIdx.x;
+  if (s >= B) return;
+  const int M = D.M, nt = D.nt, rows = M + nt, ld = nt + 1;
+  double *A = reinterpret_cast<double *>(mgs_raw);     // [rows][ld]
+  double *Rm = A + (size_t)rows * ld;                    // [nt][ld] upper triangle + transformed rhs
+  double *sc = Rm + nt * ld;                             // [nt] column scales
+  const T *resp = D.resp + (size_t)s * M * nt;
+  const T *d = D.dred + (size_t)s * M;
+  bool finite = true;
+  for (int m = lane; m < M; m += 32) {
+    const double w = D.inv_sigma[m];
+    for (int l = 0; l < nt; ++l) { const double v = (double)resp[m * nt + l] * w; A[m * ld + l] = v; finite &= isfinite(v); }
+    const double y = (double)d[m] * w;
+    A[m * ld + nt] = y;
+    finite &= isfinite(y);
+  }
+  finite = __all_sync(0xffffffffu, finite);
+  __syncwarp();
+  bool any = false;
+  for (int l = 0; l < nt; ++l) {
+    double q = 0.0;
+    for (int m = lane; m < M; m += 32) q = fma(A[m * ld + l], A[m * ld + l], q);
+    q = sqrt(warp_sum(q));
+    if (lane == 0) sc[l] = q;
+    any |= q > 0.0;
+  }
+  __syncwarp();
+  int st = !finite ? 2 : (!any ? 3 : 0);
+  const double reg = D.lambda_reg * sqrt((double)M);
+  for (int m = lane; m < M; m += 32)
+    for (int l = 0; l < nt; ++l) A[m * ld + l] = sc[l] > 0.0 ? A[m * ld + l] / sc[l] : 0.0;
+  for (int e = lane; e < nt * ld; e += 32) {             // regularisation rows; a dropped column gets a unit pivot
+    const int r = e / ld, l = e - r * ld;
+    A[(M + r) * ld + l] = (l == r) ? (sc[r] > 0.0 ? reg : 1.0) : 0.0;
+  }
+  __syncwarp();
+  double r11 = 0.0;
+  for (int l = 0; l < nt && st == 0; ++l) {
+    double q = 0.0;
+    for (int r = lane; r < rows; r += 32) q = fma(A[r * ld + l], A[r * ld + l], q);
+    const double rll = sqrt(warp_sum(q));
+    if (l == 0) r11 = rll;
+    if (!(rll > 1e-13 * r11) || !(rll > 0.0)) { st = 3; break; }
+    const double inv = 1.0 / rll;
+    for (int r = lane; r < rows; r += 32) A[r * ld + l] *= inv;
+    if (lane == 0) Rm[l * ld + l] = rll;
+    __syncwarp();
+    for (int p = l + 1; p <= nt; ++p) {
+      double dot = 0.0;
+      for (int r = lane; r < rows; r += 32) dot = fma(A[r * ld + l], A[r * ld + p], dot);
+      dot = warp_sum(dot);
+      for (int r = lane; r < rows; r += 32) A[r * ld + p] = fma(-dot, A[r * ld + l], A[r * ld + p]);
+      if (lane == 0) Rm[l * ld + p] = dot;
+    }
+    __syncwarp();
+  }
+  // back substitution R x = Q^T y (every lane redundantly, nt <= 16), then undo the column scaling
+  double X[PTEFIT_MAX_TERMS];
+  for (int l = 0; l < PTEFIT_MAX_TERMS; ++l) X[l] = 0.0;
+  if (st == 0) {
+    for (int l = nt - 1; l >= 0; --l) {
+      double v = Rm[l * ld + nt];
+      for (int p = l + 1; p < nt; ++p) v -= Rm[l * ld + p] * X[p];
+      X[l] = v / Rm[l * ld + l];
+    }
+    for (int l = 0; l < nt; ++l) X[l] = sc[l] > 0.0 ? X[l] / sc[l] : 0.0;
+  }
+  double c2 = 0.0;
+  for (int m = lane; m < M; m += 32) {
+    double rsum = -(double)d[m];
+    for (int l = 0; l < nt; ++l) rsum = fma((double)resp[m * nt + l], X[l], rsum);
+    rsum *= D.inv_sigma[m];
+    c2 = fma(rsum, rsum, c2);
+  }
+  c2 = warp_sum(c2);
+  if (lane == 0 && D.status[s] == 0) {
+    for (int l = 0; l < nt; ++l) { D.Xprev[(size_t)s * nt + l] = D.X[(size_t)s * nt + l]; D.X[(size_t)s * nt + l] = X[l]; }
+    D.chi2[s] = c2;
+    if (st != 0) D.status[s] = st;
+  }
+}
+
 // A5: node currents I = J_b X in amperes.  grid (ceil(N/256), B).
 template <typename T>
 __global__ void k_current(Dev<T> D) {

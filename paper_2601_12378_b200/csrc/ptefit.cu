@@ -391,6 +391,10 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   }
   if (ba->lsq_method != 0 && ba->lsq_method != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "lsq_method must be 0 (normal equations) or 1 (Gram-Schmidt QR)");
   if (ba->fit_coils != 0 && ba->fit_coils != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils must be 0 or 1");
+  if (ba->lsq_method == 1) {
+    const size_t sm = ((size_t)(ge->n_meas + ba->n_terms) * (ba->n_terms + 1) + (size_t)ba->n_terms * (ba->n_terms + 1) + ba->n_terms) * sizeof(double);
+    if (sm > 48 * 1024) return fail(h, PTEFIT_ERR_UNSUPPORTED, "lsq_method 1: (n_meas + n_terms)(n_terms + 1) doubles must fit 48 KB of shared memory");
+  }
   if (ba->fit_coils) {
     if (!ba->sigma_ic) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils needs sigma_ic");
     for (int c = 0; c < ge->n_coil; ++c)

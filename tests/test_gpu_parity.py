@@ -147,6 +147,22 @@ def test_cfg4_batch_subset_full_size():
     rec.close()
 
 
+@pytest.mark.parametrize("name,precision", [("cfg1", "fp64"), ("cfg2", "fp64")])
+def test_mgs_qr_driver_fp64(name, precision):
+    """lsq_method = 1 (modified Gram-Schmidt QR) against the oracle's Householder QR at the
+    FP64 tolerances; the two GPU drivers agree with each other to the conditioning of the normal equations."""
+    dev, sl = cached_case(name, 2)
+    od = oracle_device(dev)
+    n_iter = dev["meta"]["cfg"]["n_iter"]
+    rec, out = _run_gpu(dev, sl["b"], sl["ic"], n_iter, precision, lsq_method=1)
+    rec0, out0 = _run_gpu(dev, sl["b"], sl["ic"], n_iter, precision, lsq_method=0)
+    for q in range(2):
+        ores = reconstruct(od, sl["b"][q], sl["ic"][q], n_iter)
+        check_slice(out, q, ores, dev, precision)
+        assert psi_rel_err(out["psi"][q], out0["psi"][q]) <= 1e-9
+    rec.close(); rec0.close()
+
+
 def test_cfg5_reduced_fp64():
     """BASELINE config 5 grid (257x257, FP64, 76 coil columns, 4+4 terms), 2 slices, 30 iterations.
     The tension-spline edge terms of config 5 are not implemented yet (DESIGN.md gaps)."""
@@ -232,7 +248,7 @@ def test_paper_form_without_additions():
     rec.close()
 
 
-@pytest.mark.parametrize("variant", ["ffma", "nonstandard_terms", "no_graph_profiling", "solve_ffma_129", "no_fused_basis", "spline_terms"])
+@pytest.mark.parametrize("variant", ["ffma", "nonstandard_terms", "no_graph_profiling", "solve_ffma_129", "no_fused_basis", "spline_terms", "mgs_qr"])
 def test_fp32_code_path_variants(variant):
     """The FP32 path has three contraction routes and two Delta* solve routes: tcgen05 GEMM with
     in-kernel basis producer (the default, covered above), tcgen05 GEMM fed by k_basis_split (term
@@ -256,6 +272,8 @@ def test_fp32_code_path_variants(variant):
         kw = dict(flags=OPT_SOLVE_FFMA)
     if variant == "no_fused_basis":
         kw = dict(flags=OPT_NO_FUSED_BASIS)
+    if variant == "mgs_qr":
+        kw = dict(lsq_method=1)                           # the second driver of PAPER.md:116 (Gram-Schmidt QR)
     rec = _rec(dev, "fp32", 2, **kw)
     db = torch.tensor(b, dtype=rec.dtype, device="cuda"); dic = torch.tensor(ic, dtype=rec.dtype, device="cuda")
     rec.reconstruct(db, dic, n_iter)
