@@ -43,9 +43,11 @@ class Device:
         self.spline = basis.get("spline")               # dict(knots, tension, terms) or None (config 5: FF' edge terms)
         self.n_spl = 0 if self.spline is None else len(self.spline["terms"])
         self.nb = self.n_p + self.n_ff + self.n_spl + self.delz
+        self.fit_coils = int(basis.get("fit_coils", 0))   # 1 = joint fit of the coil currents, Eq. 7
+        self.sigma_ic = None if basis.get("sigma_ic") is None else np.asarray(basis["sigma_ic"], np.float64)
 
 
-def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None):
+def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None, b=None, ic=None):
     """One Picard iteration from (psin, mask).  Returns dict with X, chi2, status, psi, resp,
     I (node currents), psi_bdry and the search result `srch` of the new psi.
     X_prev: previous coefficients (for the delz column); psi_prev: flux to relax towards/from
@@ -58,8 +60,13 @@ def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None):
         col = _basis.delz_column(Jb, xp, dev.nz, dev.nr, dev.op.dz) * dev.interior
         Jb = np.concatenate([Jb, col[:, None]], axis=1)
     resp = dev.gp @ Jb                                                            # Eq. 6: R = G_P J_b
-    X, chi2, st = _lsq.fit(resp, d, dev.sigma, dev.lam)
-    out = dict(X=X, chi2=chi2, status=st, resp=resp)
+    if dev.fit_coils:                                                             # Eq. 7: coil currents fitted too,
+        X, icf, chi2, st = _lsq.fit_joint(resp, dev.gc, b, ic, dev.sigma, dev.sigma_ic, dev.lam)
+        psi_coil = (dev.ggc @ icf).reshape(dev.nz, dev.nr)                        # and the coil flux follows them
+        out = dict(X=X, chi2=chi2, status=st, resp=resp, ic_fit=icf)
+    else:
+        X, chi2, st = _lsq.fit(resp, d, dev.sigma, dev.lam)
+        out = dict(X=X, chi2=chi2, status=st, resp=resp)
     if st != 0:
         return out
     I = Jb @ X                                                                    # J_phi dA = J_b X
@@ -97,12 +104,15 @@ def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False):
             break
         have_prev = (psi0 is not None) or it > 0     # cold start: the first flux is taken as is
         o = picard_iteration(dev, psin, mask, d, psi_coil, X_prev=res["X"],
-                             psi_prev=res["psi"] if have_prev else None)
+                             psi_prev=res["psi"] if have_prev else None, b=np.asarray(b, np.float64), ic=np.asarray(ic, np.float64))
+        if "ic_fit" in o:
+            res["ic_fit"] = o["ic_fit"]
         res["X"], res["chi2"], res["status"] = o["X"], o["chi2"], o["status"]
         if "psi" in o:
             if trace:
                 res["hist"].append(dict(X=o["X"], chi2=o["chi2"], dpsi=float(np.max(np.abs(o["psi"] - res["psi"]))),
-                                        psi=o["psi"], resp=o["resp"], I=o["I"], psi_bdry=o["psi_bdry"], srch=o["srch"]))
+                                        psi=o["psi"], resp=o["resp"], I=o["I"], psi_bdry=o["psi_bdry"], srch=o["srch"],
+                                        ic_fit=o.get("ic_fit")))
             res["psi"], res["srch"] = o["psi"], o["srch"]
             psin, mask = o["srch"]["psin"], o["srch"]["mask"]
     return res
