@@ -88,7 +88,9 @@ typedef struct {
   int lsq_method;              /* 0 = normal equations + Cholesky, 1 = modified Gram-Schmidt QR
                                   (the two drivers of PAPER.md:116)                             */
   int fit_coils;               /* 1 = joint fit of the coil currents, Eq. 7:
-                                  unknowns [X; I_C'], extra rows I_C' = I_C weighted 1/sigma_ic  */
+                                  unknowns [X; I_C'], extra rows I_C' = I_C weighted 1/sigma_ic; the coil
+                                  flux G_GC I_C' is recomputed every iteration; chi2 = measurement rows;
+                                  needs n_terms + n_coil <= 96 and lsq_method 0                   */
   const double *sigma_ic;      /* [n_coil] HOST, 1-sigma of the measured coil currents (fit_coils) */
 } ptefit_basis;
 
@@ -169,6 +171,10 @@ int ptefit_last_launch_count(const ptefit_handle *h);
  * Synchronises the stream. */
 ptefit_status ptefit_set_profiling(ptefit_handle *h, int on);
 ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
+
+/* Fitted coil currents I_C' of the last reconstruct call of a handle created with fit_coils = 1 (Eq. 7,
+ * PAPER.md:87-93): d_out[batch][n_coil] real, DEVICE.  Asynchronous on cuda_stream. */
+ptefit_status ptefit_get_coil_currents(ptefit_handle *h, int batch, void *d_out, void *cuda_stream);
 
 /* NEXT-3: a Green's table on the GPU (Sec. II.A, Eq. 3-5; closed forms
  * with complete elliptic integrals, reading O1 of DESIGN.md).  out[k][c] = w_c g(field point k, source c)

@@ -11,7 +11,7 @@ LIB_PATH = os.path.join(HERE, "libptefit.so")
 EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
-    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table",
+    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table", "ptefit_get_coil_currents",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
@@ -90,6 +90,8 @@ def load_library():
         lib.ptefit_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.ptefit_get_stage_ms.restype = C.c_int
         lib.ptefit_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        lib.ptefit_get_coil_currents.restype = C.c_int
+        lib.ptefit_get_coil_currents.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         lib.ptefit_greens_table.restype = C.c_int
         lib.ptefit_greens_table.argtypes = ([C.c_int] + [C.c_void_p] * 4 + [C.c_int] + [C.c_void_p] * 4 + [C.c_int, C.c_void_p])
         _lib = lib
@@ -256,6 +258,13 @@ class Reconstructor:
         s = self.torch.cuda.current_stream()
         self._call(self.lib.ptefit_debug_fit, d_xn.shape[0], _dp(d_xn), _dp(d_b), _dp(d_ic), _dp(d_xprev), _dp(d_resp),
                    _dp(self.coeffs), _dp(self.chi2), _dp(self.status), C.c_void_p(s.cuda_stream))
+
+    def coil_currents(self, B):
+        """Fitted coil currents of the last call (fit_coils = 1): torch tensor [B, n_coil]."""
+        out = self.torch.zeros(B, self.nc, dtype=self.dtype, device="cuda")
+        s = self.torch.cuda.current_stream()
+        self._call(self.lib.ptefit_get_coil_currents, B, _dp(out), C.c_void_p(s.cuda_stream))
+        return out
 
     def launch_count(self):
         return self.lib.ptefit_last_launch_count(self.h)

@@ -54,6 +54,9 @@ struct Dev {
   int nr, nz, N, nri, nzi, nbnd, M, nc, nt, npoly, has_delz, nlim, ip_sign;
   int nspl, maxdeg;               // spline terms among the npoly basis terms; largest polynomial exponent
   int lsq_method;                 // 0 normal equations + Cholesky, 1 modified Gram-Schmidt
+  int fit_coils;                  // 1 = joint fit of the coil currents, Eq. 7 (joint_fit.cuh)
+  const double *gcw, *c22s, *tcoil, *inv_sic2;   // W G_C [M][nc]; scaled G_C^T W^2 G_C + diag(1/sigma_ic^2) [nc][nc]; column scales; 1/sigma_ic^2
+  double *icf, *icm;              // [B][nc] fitted / measured coil currents
   const SplineDev *spl;           // nullptr unless nspl > 0
   const CallArgs *ca;             // device copy of the caller's pointers (k_set_args)
   double rmin, zmin, dr, dz, dA, lambda_reg, relax;

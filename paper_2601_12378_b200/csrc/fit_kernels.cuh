@@ -28,8 +28,13 @@ __global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__
     const T *g = D.gc + (size_t)m * D.nc;
     T acc = T(0);
     for (int c = 0; c < D.nc; ++c) acc = fma(g[c], sic[c], acc);
-    D.dred[(size_t)s * D.M + m] = b[(size_t)s * D.M + m] - acc;
+    D.dred[(size_t)s * D.M + m] = D.fit_coils ? b[(size_t)s * D.M + m] : b[(size_t)s * D.M + m] - acc;   // Eq. 7 fits b itself
   }
+  if (D.fit_coils)
+    for (int c = n; c < D.nc; c += gridDim.x * blockDim.x) {
+      const double v = (double)ic[(size_t)s * D.nc + c];
+      D.icm[(size_t)s * D.nc + c] = v; D.icf[(size_t)s * D.nc + c] = v;
+    }
   if (n < D.nt) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
   if (n == 0) { D.status[s] = 0; D.chi2[s] = 0.0; }
 }

@@ -22,6 +22,7 @@
 #include "dmma_gemm.cuh"
 #include "dmma_kernels.cuh"
 #include "greens_kernels.cuh"
+#include "joint_fit.cuh"
 
 using namespace ptefit;
 
@@ -127,7 +128,7 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   D.dr = (g->rmax - g->rmin) / (g->nr - 1); D.dz = (g->zmax - g->zmin) / (g->nz - 1);
   D.dA = D.dr * D.dz; D.lambda_reg = ba->lambda_reg; D.relax = ba->relax;
   D.cold_rc = ge->cold_rc; D.cold_zc = ge->cold_zc; D.cold_a = ge->cold_a; D.cold_b = ge->cold_b;
-  D.npoly = 0; D.has_delz = 0; D.nspl = 0; D.maxdeg = 0; D.spl = nullptr; D.lsq_method = ba->lsq_method;
+  D.npoly = 0; D.has_delz = 0; D.nspl = 0; D.maxdeg = 0; D.spl = nullptr; D.lsq_method = ba->lsq_method; D.fit_coils = ba->fit_coils;
   const ptefit_term *spl_term = nullptr;
   for (int l = 0; l < ba->n_terms; ++l) {
     const ptefit_term &t = ba->terms[l];
@@ -198,6 +199,32 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
     std::vector<double> w(D.M);
     for (int m = 0; m < D.M; ++m) w[m] = 1.0 / ge->sigma[m];
     TRY(upload(h, &D.inv_sigma, w.data(), w.size()));
+  }
+  if (ba->fit_coils) {
+    // constants of the joint fit (Eq. 7): W G_C, and the coil-coil block G_C^T W^2 G_C + diag(1/sigma_ic^2)
+    // scaled to a unit diagonal, FP64, from the table values the kernels see (rounded to T first)
+    const int M = D.M, nc = D.nc;
+    std::vector<double> gw((size_t)M * nc), c22((size_t)nc * nc, 0.0), tc(nc), is2(nc);
+    for (int m = 0; m < M; ++m)
+      for (int c = 0; c < nc; ++c) gw[(size_t)m * nc + c] = (double)(T)tb->gc[(size_t)m * nc + c] / ge->sigma[m];
+    for (int c = 0; c < nc; ++c) is2[c] = 1.0 / (ba->sigma_ic[c] * ba->sigma_ic[c]);
+    for (int c = 0; c < nc; ++c)
+      for (int e = 0; e <= c; ++e) {
+        double acc = 0.0;
+        for (int m = 0; m < M; ++m) acc += gw[(size_t)m * nc + c] * gw[(size_t)m * nc + e];
+        if (e == c) acc += is2[c];
+        c22[(size_t)c * nc + e] = c22[(size_t)e * nc + c] = acc;
+      }
+    for (int c = 0; c < nc; ++c) tc[c] = sqrt(c22[(size_t)c * nc + c]);
+    for (int c = 0; c < nc; ++c)
+      for (int e = 0; e < nc; ++e) c22[(size_t)c * nc + e] /= tc[c] * tc[e];
+    TRY(upload(h, &D.gcw, gw.data(), gw.size()));
+    TRY(upload(h, &D.c22s, c22.data(), c22.size()));
+    TRY(upload(h, &D.tcoil, tc.data(), tc.size()));
+    TRY(upload(h, &D.inv_sic2, is2.data(), is2.size()));
+    TRY(dev_alloc(h, &D.icf, (size_t)B * nc));
+    TRY(dev_alloc(h, &D.icm, (size_t)B * nc));
+    CK(cudaFuncSetAttribute(k_lsq_joint<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)joint_smem_bytes(M, D.nt, nc)));
   }
   TRY(upload(h, &D.lim_mask, ge->lim_mask, N));
   TRY(upload(h, &D.xpt_mask, ge->xpt_mask ? ge->xpt_mask : ge->lim_mask, N));
@@ -399,6 +426,9 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
     if (!ba->sigma_ic) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils needs sigma_ic");
     for (int c = 0; c < ge->n_coil; ++c)
       if (!(ba->sigma_ic[c] > 0.0)) return fail(h, PTEFIT_ERR_INVALID_ARG, "sigma_ic must be > 0");
+    if (ba->n_terms + ge->n_coil > JOINT_MAX_N || joint_smem_bytes(ge->n_meas, ba->n_terms, ge->n_coil) > 200 * 1024)
+      return fail(h, PTEFIT_ERR_UNSUPPORTED, "fit_coils: n_terms + n_coil must be <= 96 and the normal matrix must fit 200 KB of shared memory");
+    if (ba->lsq_method != 0) return fail(h, PTEFIT_ERR_UNSUPPORTED, "fit_coils uses the normal-equation driver (lsq_method 0)");
   }
   if (op->gemm != PTEFIT_GEMM_3XTF32 && op->gemm != PTEFIT_GEMM_FFMA) return fail(h, PTEFIT_ERR_INVALID_ARG, "gemm must be PTEFIT_GEMM_3XTF32 or PTEFIT_GEMM_FFMA");
   if (op->flags & ~(PTEFIT_OPT_NO_GRAPH | PTEFIT_OPT_NO_FUSED_BASIS | PTEFIT_OPT_SOLVE_FFMA)) return fail(h, PTEFIT_ERR_INVALID_ARG, "unknown option flag");
@@ -451,6 +481,17 @@ extern "C" ptefit_status ptefit_greens_table(int n_fld, const double *fr, const 
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(h, PTEFIT_ERR_CUDA, "no CUDA device (there is no CPU fallback)");
   k_greens_table<<<dim3((n_src + 255) / 256, n_fld), 256, 0, (cudaStream_t)cuda_stream>>>(n_fld, fr, fz, fcos, fsin, n_src, sr, sz, sw, out,
                                                                                         transpose ? 1 : 0);
+  CK(cudaGetLastError());
+  return PTEFIT_OK;
+}
+
+extern "C" ptefit_status ptefit_get_coil_currents(ptefit_handle *h, int batch, void *d_out, void *cuda_stream) {
+  if (!h || !d_out || batch < 1 || batch > h->max_batch) return fail(h, PTEFIT_ERR_INVALID_ARG, "ptefit_get_coil_currents: bad arguments");
+  const bool on = h->prec == PTEFIT_FP32 ? h->d32.fit_coils : h->d64.fit_coils;
+  if (!on) return fail(h, PTEFIT_ERR_INVALID_ARG, "ptefit_get_coil_currents: the handle was created without fit_coils");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->prec == PTEFIT_FP32) k_export_ic<float><<<(batch * h->d32.nc + 255) / 256, 256, 0, st>>>(h->d32, batch, (float *)d_out);
+  else k_export_ic<double><<<(batch * h->d64.nc + 255) / 256, 256, 0, st>>>(h->d64, batch, (double *)d_out);
   CK(cudaGetLastError());
   return PTEFIT_OK;
 }

@@ -163,6 +163,32 @@ def test_mgs_qr_driver_fp64(name, precision):
     rec.close(); rec0.close()
 
 
+@pytest.mark.parametrize("name,precision,ns", [("cfg1", "fp64", 2), ("cfg2", "fp32", 2), ("cfg4", "fp32", 6)])
+def test_joint_coil_fit_eq7(name, precision, ns):
+    """NEXT-1: joint fit of the coil currents (Eq. 7).  The measured currents handed to both
+    sides are the generator's currents with seeded 3 % errors; the fitted currents, coefficients and flux
+    must match the oracle's fit_joint loop (cfg4: 76 coil columns + 7 terms = 83 unknowns per slice)."""
+    torch = _torch()
+    dev, sl = cached_case(name, ns)
+    rng = np.random.default_rng(17)
+    sic = np.full(sl["ic"].shape[1], 0.03) * np.maximum(np.abs(sl["ic"]).max(axis=0), 1.0)
+    meas = sl["ic"] + sic[None, :] * rng.standard_normal(sl["ic"].shape)
+    dj = dict(dev); dj["basis"] = dict(dev["basis"], fit_coils=1, sigma_ic=sic)
+    dv, b, ic = round_inputs(dj, dict(b=sl["b"], ic=meas), precision)
+    od = oracle_device(dv)
+    n_iter = dev["meta"]["cfg"]["n_iter"]
+    rec, out = _run_gpu(dj, b, ic, n_iter, precision, fit_coils=1, sigma_ic=sic)
+    icf = rec.coil_currents(ns).cpu().numpy().astype(np.float64)
+    for q in range(ns):
+        ores = reconstruct(od, b[q], ic[q], n_iter)
+        assert ores["status"] == 0
+        check_slice(out, q, ores, dj, precision, strict_index=(precision == "fp64"))
+        tol = 1e-4 if precision == "fp32" else 1e-9
+        assert np.max(np.abs(icf[q] - ores["ic_fit"])) <= tol * np.max(np.abs(ores["ic_fit"])), q
+        assert np.max(np.abs(ores["ic_fit"] - ic[q])) > 1e-3 * np.max(np.abs(ic[q]))      # the fit did move the currents
+    rec.close()
+
+
 def test_cfg5_reduced_fp64():
     """BASELINE config 5 grid (257x257, FP64, 76 coil columns, 4+4 terms), 2 slices, 30 iterations.
     The tension-spline edge terms of config 5 are not implemented yet (DESIGN.md gaps)."""
