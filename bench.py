@@ -413,16 +413,27 @@ def latency_batch1(args, torch, P):
     d_b8 = torch.tensor(sl8["b"], dtype=rec.dtype, device="cuda")
     d_ic8 = torch.tensor(sl8["ic"], dtype=rec.dtype, device="cuda")
     n_stream = 10000
+    # slow flux variation: the measurements drift linearly from one stored equilibrium to the
+    # next over 1250 slices
+    seg = n_stream // 8
+    al = (torch.arange(n_stream, device="cuda") % seg).to(rec.dtype)[:, None] / seg
+    k0 = (torch.arange(n_stream, device="cuda") // seg) % 8
+    k1 = (k0 + 1) % 8
+    b_all = d_b8[k0] * (1 - al) + d_b8[k1] * al
+    ic_all = d_ic8[k0] * (1 - al) + d_ic8[k1] * al
+    rec.reconstruct(b_all[0:1], ic_all[0:1], c["n_iter"])      # converge on the first slice, then stream
+    n_ok = 0
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(n_stream + 1)]
+    stat = torch.zeros(n_stream, dtype=torch.int32, device="cuda")
     evs[0].record()
     for q in range(n_stream):
-        k = (q // 250) % 8                                   # the equilibrium changes every 250 slices
-        rec.reconstruct(d_b8[k:k + 1], d_ic8[k:k + 1], 1, warm_start=True)
+        rec.reconstruct(b_all[q:q + 1], ic_all[q:q + 1], 1, warm_start=True)
         evs[q + 1].record()
+        stat[q:q + 1].copy_(rec.status[0:1], non_blocking=True)    # outside the event pair of slice q, inside that of q + 1
     torch.cuda.synchronize()
     st = np.array([evs[q].elapsed_time(evs[q + 1]) for q in range(n_stream)]) * 1e3
     stream = dict(slices=n_stream, us_mean=float(st.mean()), us_p50=float(np.percentile(st, 50)), us_p99=float(np.percentile(st, 99)),
-                  us_max=float(st.max()), status_ok=int(rec.status[0].item() == 0),
+                  us_max=float(st.max()), status_ok=int((stat == 0).sum().item()),
                   note="one warm-started Picard iteration per slice, back-to-back launches, no post-processing")
     rec.close()
     return dict(workload="cfg3", streaming=stream, us_per_slice=1e3 * float(np.median(ts)), us_min=1e3 * float(min(ts)), n_iter=c["n_iter"],

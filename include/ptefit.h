@@ -172,6 +172,27 @@ int ptefit_last_launch_count(const ptefit_handle *h);
 ptefit_status ptefit_set_profiling(ptefit_handle *h, int on);
 ptefit_status ptefit_get_stage_ms(ptefit_handle *h, float out[6]);
 
+/* NEXT-2: flux-surface post-processing of the last ptefit_reconstruct call of this handle
+ * (Sec. II.E, Eq. 12, Fig. 1; readings in DESIGN.md O8).  For n_prof levels
+ * x_p = (p + 1)/n_prof of the normalised flux and n_chord chords from the refined axis (angles 2 pi c/n_chord,
+ * counter-clockwise) the vertex of every flux surface on every chord is found by n_bisect bisection steps
+ * (the paper uses about 10) plus one linear interpolation; then Q_{mu,nu} = closed integral of
+ * |grad psi|^mu R^nu dl (trapezoid rule on the vertex polygon) for the n_q <= 8 exponent pairs given,
+ * q = (mu0 F / 2 pi) Q_{-1,-1} (NaN unless that pair is listed; F from f_vac and the fitted FF' polynomial),
+ * and the geometry of the last level (LCFS): R_min, R_max, Z_min, Z_max, minor radius, elongation.
+ * d_psi must be the flux that reconstruct call returned.  Outputs, DEVICE, real: d_Q[batch][n_prof][n_q],
+ * d_q[batch][n_prof], d_geom[batch][6], d_vert[batch][n_prof][n_chord][2] (may be NULL),
+ * d_status[batch] (may be NULL; 1 = slice failed or its axis lies outside the plasma).
+ * Limits: n_prof * n_chord <= 12288, n_chord <= 1024.  Asynchronous on cuda_stream. */
+typedef struct {
+  int n_prof, n_chord, n_bisect;
+  int n_q;
+  const int *mu, *nu;            /* HOST [n_q] */
+  double f_vac;                  /* vacuum R B_phi / mu0 in amperes (the paper's F at the boundary) */
+} ptefit_profile_spec;
+ptefit_status ptefit_flux_surfaces(ptefit_handle *h, int batch, const ptefit_profile_spec *spec, const void *d_psi,
+                                   void *d_Q, void *d_q, void *d_geom, void *d_vert, int *d_status, void *cuda_stream);
+
 /* Fitted coil currents I_C' of the last reconstruct call of a handle created with fit_coils = 1 (Eq. 7,
  * PAPER.md:87-93): d_out[batch][n_coil] real, DEVICE.  Asynchronous on cuda_stream. */
 ptefit_status ptefit_get_coil_currents(ptefit_handle *h, int batch, void *d_out, void *cuda_stream);

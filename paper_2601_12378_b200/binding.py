@@ -11,7 +11,7 @@ LIB_PATH = os.path.join(HERE, "libptefit.so")
 EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
-    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table", "ptefit_get_coil_currents",
+    "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table", "ptefit_get_coil_currents", "ptefit_flux_surfaces",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
@@ -48,6 +48,11 @@ class _Term(C.Structure):
 class _Basis(C.Structure):
     _fields_ = [("n_terms", C.c_int), ("terms", C.POINTER(_Term)), ("lambda_reg", C.c_double), ("relax", C.c_double),
                 ("lsq_method", C.c_int), ("fit_coils", C.c_int), ("sigma_ic", C.c_void_p)]
+
+
+class _ProfileSpec(C.Structure):
+    _fields_ = [("n_prof", C.c_int), ("n_chord", C.c_int), ("n_bisect", C.c_int), ("n_q", C.c_int), ("mu", C.c_void_p),
+                ("nu", C.c_void_p), ("f_vac", C.c_double)]
 
 
 class _Options(C.Structure):
@@ -90,6 +95,8 @@ def load_library():
         lib.ptefit_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.ptefit_get_stage_ms.restype = C.c_int
         lib.ptefit_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        lib.ptefit_flux_surfaces.restype = C.c_int
+        lib.ptefit_flux_surfaces.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 8
         lib.ptefit_get_coil_currents.restype = C.c_int
         lib.ptefit_get_coil_currents.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         lib.ptefit_greens_table.restype = C.c_int
@@ -258,6 +265,20 @@ class Reconstructor:
         s = self.torch.cuda.current_stream()
         self._call(self.lib.ptefit_debug_fit, d_xn.shape[0], _dp(d_xn), _dp(d_b), _dp(d_ic), _dp(d_xprev), _dp(d_resp),
                    _dp(self.coeffs), _dp(self.chi2), _dp(self.status), C.c_void_p(s.cuda_stream))
+
+    def flux_surfaces(self, B, n_prof=33, n_chord=128, n_bisect=10, munu=((-1, -1), (-1, -2), (0, 0)), f_vac=0.0, want_vert=True):
+        """Flux-surface post-processing of the last reconstruct call (ptefit_flux_surfaces).  Returns a dict of
+        torch tensors Q[B, n_prof, n_q], q[B, n_prof], geom[B, 6], vert[B, n_prof, n_chord, 2], status[B]."""
+        t = self.torch
+        mu = np.ascontiguousarray([m for m, _ in munu], np.int32); nu = np.ascontiguousarray([n for _, n in munu], np.int32)
+        sp = _ProfileSpec(int(n_prof), int(n_chord), int(n_bisect), len(munu), _ptr(mu), _ptr(nu), float(f_vac))
+        kw = dict(dtype=self.dtype, device="cuda")
+        out = dict(Q=t.zeros(B, n_prof, len(munu), **kw), q=t.zeros(B, n_prof, **kw), geom=t.zeros(B, 6, **kw),
+                   vert=t.zeros(B, n_prof, n_chord, 2, **kw) if want_vert else None, status=t.zeros(B, dtype=t.int32, device="cuda"))
+        s = t.cuda.current_stream()
+        self._call(self.lib.ptefit_flux_surfaces, B, C.byref(sp), _dp(self.psi), _dp(out["Q"]), _dp(out["q"]), _dp(out["geom"]),
+                   _dp(out["vert"]), _dp(out["status"]), C.c_void_p(s.cuda_stream))
+        return out
 
     def coil_currents(self, B):
         """Fitted coil currents of the last call (fit_coils = 1): torch tensor [B, n_coil]."""

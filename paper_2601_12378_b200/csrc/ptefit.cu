@@ -23,6 +23,7 @@
 #include "dmma_kernels.cuh"
 #include "greens_kernels.cuh"
 #include "joint_fit.cuh"
+#include "fluxsurf_kernels.cuh"
 
 using namespace ptefit;
 
@@ -483,6 +484,38 @@ extern "C" ptefit_status ptefit_greens_table(int n_fld, const double *fr, const 
                                                                                         transpose ? 1 : 0);
   CK(cudaGetLastError());
   return PTEFIT_OK;
+}
+
+namespace {
+template <typename T>
+ptefit_status flux_surfaces(ptefit_handle *h, Dev<T> &D, int B, const ptefit_profile_spec *sp, const T *psi, T *Q, T *q, T *geom, T *vert,
+                            int *fstat, cudaStream_t st) {
+  FsSpec S{};
+  S.n_prof = sp->n_prof; S.n_chord = sp->n_chord; S.n_bisect = sp->n_bisect; S.n_q = sp->n_q; S.f_vac = sp->f_vac; S.q_index = -1;
+  for (int e = 0; e < sp->n_q; ++e) { S.mu[e] = sp->mu[e]; S.nu[e] = sp->nu[e]; if (sp->mu[e] == -1 && sp->nu[e] == -1) S.q_index = e; }
+  S.ff0 = -1; S.n_ff = 0;
+  for (int l = 0; l < D.nt; ++l)
+    if (D.terms[l].kind == 1 && D.terms[l].family == 0) { if (S.ff0 < 0) S.ff0 = l; S.n_ff++; }
+  if (S.ff0 < 0) S.ff0 = 0;
+  const size_t sm = ((size_t)S.n_chord + 2 * (size_t)S.n_prof * S.n_chord) * sizeof(double);
+  CK(cudaFuncSetAttribute(k_flux_surfaces<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+  k_flux_surfaces<T><<<B, FS_THREADS, sm, st>>>(D, S, psi, Q, q, geom, vert, fstat);
+  CK(cudaGetLastError());
+  return PTEFIT_OK;
+}
+}  // namespace
+
+extern "C" ptefit_status ptefit_flux_surfaces(ptefit_handle *h, int batch, const ptefit_profile_spec *sp, const void *d_psi, void *d_Q,
+                                              void *d_q, void *d_geom, void *d_vert, int *d_status, void *cuda_stream) {
+  if (!h || !sp || !d_psi || !d_Q || !d_q || !d_geom || batch < 1 || batch > h->max_batch)
+    return fail(h, PTEFIT_ERR_INVALID_ARG, "ptefit_flux_surfaces: bad arguments");
+  if (sp->n_prof < 1 || sp->n_chord < 3 || sp->n_chord > 1024 || (long long)sp->n_prof * sp->n_chord > 12288 || sp->n_bisect < 0 || sp->n_bisect > 60 ||
+      sp->n_q < 1 || sp->n_q > FS_MAX_Q || !sp->mu || !sp->nu)
+    return fail(h, PTEFIT_ERR_INVALID_ARG, "ptefit_flux_surfaces: need 1 <= n_prof, 3 <= n_chord <= 1024, n_prof n_chord <= 12288, 0 <= n_bisect <= 60, 1 <= n_q <= 8");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (h->prec == PTEFIT_FP32)
+    return flux_surfaces<float>(h, h->d32, batch, sp, (const float *)d_psi, (float *)d_Q, (float *)d_q, (float *)d_geom, (float *)d_vert, d_status, st);
+  return flux_surfaces<double>(h, h->d64, batch, sp, (const double *)d_psi, (double *)d_Q, (double *)d_q, (double *)d_geom, (double *)d_vert, d_status, st);
 }
 
 extern "C" ptefit_status ptefit_get_coil_currents(ptefit_handle *h, int batch, void *d_out, void *cuda_stream) {

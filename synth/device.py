@@ -24,7 +24,7 @@ CONFIGS = {
                  shapes=("limited", "limited", "lsn", "usn", "dn")),
 }
 RMIN, RMAX = 0.15, 1.60
-LAMBDA_REG = 0.003
+LAMBDA_REG = 0.005
 RELAX = 0.6
 
 

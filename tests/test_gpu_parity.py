@@ -452,8 +452,8 @@ def test_response_fit_full_batch_cfg4():
     dev, sl = cached_case("cfg4", 24)
     dv, b, ic = round_inputs(dev, sl, "fp32")
     od = oracle_device(dv)
-    ores = [reconstruct(od, b[q], ic[q], 3, trace=True) for q in range(24)]
-    hk = [o["hist"][2] for o in ores]; prev = [o["hist"][1] for o in ores]
+    ores = [reconstruct(od, b[q], ic[q], 6, trace=True) for q in range(24)]
+    hk = [o["hist"][5] for o in ores]; prev = [o["hist"][4] for o in ores]
     rec = _rec(dev, "fp32", 512)
     dt = rec.dtype
     til = lambda a: np.tile(a, (22,) + (1,) * (a.ndim - 1))[:512]
@@ -464,11 +464,25 @@ def test_response_fit_full_batch_cfg4():
     torch.cuda.synchronize()
     r = resp.cpu().numpy().astype(np.float64)
     X = rec.coeffs.cpu().numpy().astype(np.float64)
+    # the oracle's response and fit on exactly what the GPU stage was given: normalised flux and previous
+    # coefficients rounded to FP32 (a 6e-8 change of psi_N moves the coefficients of this ill-conditioned fit
+    # by more than the GEMM does, so the stage is compared on identical inputs)
+    ref = []
+    for k in range(24):
+        x32 = xin[k].astype(np.float32).astype(np.float64).reshape(od.nz, od.nr)
+        m32 = x32 >= 0
+        Jb = OB.basis_columns(np.where(m32, x32, 0.0), m32, od.r, od.dA, od.n_p, od.n_ff).reshape(-1, od.n_p + od.n_ff) * od.interior[:, None]
+        xp = prev[k]["X"].astype(np.float32).astype(np.float64)[:od.n_p + od.n_ff]
+        col = OB.delz_column(Jb, xp, od.nz, od.nr, od.op.dz) * od.interior
+        r_or = od.gp @ np.concatenate([Jb, col[:, None]], axis=1)
+        X_or, _, st = OL.fit(r_or, b[k] - od.gc @ ic[k], od.sigma, od.lam)
+        assert st == 0
+        ref.append((r_or, X_or))
     for q in range(512):
-        r_or = hk[q % 24]["resp"]
+        r_or, X_or = ref[q % 24]
         cs = np.max(np.abs(r_or), axis=0)
         assert np.max(np.abs(r[q] - r_or) / cs) <= 5e-6, q
-        assert coef_rel_err(X[q], hk[q % 24]["X"], od.n_p, od.n_ff, od.op.dz) <= 1e-4, q
+        assert coef_rel_err(X[q], X_or, od.n_p, od.n_ff, od.op.dz) <= 1e-4, q
         if q >= 24:
             assert np.array_equal(r[q], r[q % 24]) and np.array_equal(X[q], X[q % 24])
     rec.close()
