@@ -25,10 +25,12 @@ __global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__
     D.psi_coil[(size_t)s * D.N + n] = acc;
   }
   for (int m = n; m < D.M; m += gridDim.x * blockDim.x) {       // M may exceed the node count of a small grid
+    // FP64 accumulation: b and G_C I_C nearly cancel when the coil signal dominates the plasma signal, and an
+    // FP32 sum of n_c terms would leave d with a relative error of ~1e-6 |G_C I_C| / |d|
     const T *g = D.gc + (size_t)m * D.nc;
-    T acc = T(0);
-    for (int c = 0; c < D.nc; ++c) acc = fma(g[c], sic[c], acc);
-    D.dred[(size_t)s * D.M + m] = D.fit_coils ? b[(size_t)s * D.M + m] : b[(size_t)s * D.M + m] - acc;   // Eq. 7 fits b itself
+    double acc = 0.0;
+    for (int c = 0; c < D.nc; ++c) acc = fma((double)g[c], (double)sic[c], acc);
+    D.dred[(size_t)s * D.M + m] = D.fit_coils ? b[(size_t)s * D.M + m] : T((double)b[(size_t)s * D.M + m] - acc);   // Eq. 7 fits b itself
   }
   if (D.fit_coils)
     for (int c = n; c < D.nc; c += gridDim.x * blockDim.x) {
