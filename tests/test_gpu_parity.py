@@ -491,3 +491,58 @@ def test_response_fit_full_batch_cfg4():
         if q >= 24:
             assert np.array_equal(r[q], r[q % 24]) and np.array_equal(X[q], X[q % 24])
     rec.close()
+
+
+@pytest.mark.parametrize("n,precision", [(9, "fp32"), (9, "fp64"), (17, "fp32"), (17, "fp64"), (33, "fp32")])
+def test_small_grids_solve_stage(n, precision):
+    """Smallest grids the header allows (9x9, 17x17): the Delta* solve stage against the oracle's banded LU
+    (the twisted-Thomas hand-over buffer must fit the shared memory of small grids)."""
+    torch = _torch()
+    from oracle.gs_solve import GSOperator, boundary_nodes
+    import paper_2601_12378_b200 as P
+    rng = np.random.default_rng(n)
+    grid = dict(nr=n, nz=n, rmin=0.15, rmax=1.6, zmin=-1.5, zmax=1.5)
+    op = GSOperator(n, n, 0.15, 1.6, -1.5, 1.5)
+    bnd = boundary_nodes(n, n)
+    lim = np.zeros((n, n), np.uint8); lim[2:-2, 2:-2] = 1
+    M, nc = 6, 3
+    geom = dict(n_meas=M, n_coil=nc, sigma=np.ones(M), lim_r=np.array([0.5, 1.2, 0.9]), lim_z=np.array([-0.5, 0.0, 0.6]), lim_mask=lim,
+                xpt_mask=None, ip_sign=1, cold_rc=0.8, cold_zc=0.0, cold_a=0.4, cold_b=0.7)
+    tables = dict(gp=rng.normal(size=(M, n * n)), gc=rng.normal(size=(M, nc)), gb=rng.normal(size=(len(bnd), n * n)) * 1e-7,
+                  ggc=rng.normal(size=(n * n, nc)) * 1e-7)
+    dev = dict(grid=grid, geom=geom, tables=tables, basis=dict(n_p=1, n_ff=1, lambda_reg=0.01, relax=1.0, delz=0))
+    B = 5
+    rec = P.Reconstructor(dev, precision=precision, max_batch=B)
+    npdt = np.float32 if precision == "fp32" else np.float64
+    I = (rng.uniform(0.0, 40.0, (B, n * n)) * lim.ravel()[None, :]).astype(npdt)
+    pbd = rng.uniform(-0.05, 0.05, (B, len(bnd))).astype(npdt)
+    out = torch.zeros(B, n, n, dtype=rec.dtype, device="cuda")
+    rec.debug_gs_solve(torch.tensor(I, device="cuda"), torch.tensor(pbd, device="cuda"), out)
+    psi = out.cpu().numpy().astype(np.float64)
+    for q in range(B):
+        edge = np.zeros(n * n); edge[bnd] = pbd[q].astype(np.float64)
+        ref = op.solve_current(I[q].astype(np.float64).reshape(n, n), edge.reshape(n, n))
+        assert psi_rel_err(psi[q], ref) <= PSI_TOL[precision], (n, precision, q)
+    rec.close()
+
+
+def test_large_batch_beyond_one_wave_of_row_tiles():
+    """batches whose response GEMM needs more than 148 row tiles (B > 2368 at 8 rows per
+    slice) must stay inside the split-K partial buffers.  B = 2500 on config 2: the 8 stored slices tiled
+    over the batch; replicas bit-identical, the first 8 against the oracle."""
+    torch = _torch()
+    dev, sl = cached_case("cfg2", 8)
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    od = oracle_device(dv)
+    B = 2500
+    rec = _rec(dev, "fp32", B)
+    bb = np.tile(b, (B // 8 + 1, 1))[:B]; icc = np.tile(ic, (B // 8 + 1, 1))[:B]
+    rec.reconstruct(torch.tensor(bb, dtype=rec.dtype, device="cuda"), torch.tensor(icc, dtype=rec.dtype, device="cuda"), 15)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, B)
+    for q in range(8):
+        ores = reconstruct(od, b[q], ic[q], 15)
+        check_slice(out, q, ores, dev, "fp32", strict_index=False)
+    for q in range(8, B):
+        assert np.array_equal(out["psi"][q], out["psi"][q % 8]) and np.array_equal(out["coeffs"][q], out["coeffs"][q % 8]), q
+    rec.close()
