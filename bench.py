@@ -412,7 +412,7 @@ def latency_batch1(args, torch, P):
     dev8, sl8 = make_workload("cfg3", 8)
     d_b8 = torch.tensor(sl8["b"], dtype=rec.dtype, device="cuda")
     d_ic8 = torch.tensor(sl8["ic"], dtype=rec.dtype, device="cuda")
-    n_stream = 10000
+    n_stream = 400 if args.latency_only else 10000
     # slow flux variation: the measurements drift linearly from one stored equilibrium to the
     # next over 1250 slices
     seg = n_stream // 8
@@ -455,8 +455,13 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=24, help="slices the cpu_baseline leg times")
     ap.add_argument("--skip-extras", action="store_true", help="timed region + stage breakdown only (for ncu runs)")
     ap.add_argument("--ref-sample", type=int, default=4, help="--impl reference: slices per step")
+    ap.add_argument("--latency-only", action="store_true", help="only the batch-1 latency section (cfg3), for ncu launch lists")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.latency_only:
+        import torch
+        import paper_2601_12378_b200 as P
+        print(json.dumps(dict(latency_batch1=latency_batch1(args, torch, P))), flush=True)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
