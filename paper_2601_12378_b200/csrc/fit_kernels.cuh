@@ -144,6 +144,10 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
   const T *resp = D.resp + (size_t)s * D.M * nt;
   const T *d = D.dred + (size_t)s * D.M;
   constexpr int NA = NT * (NT + 1) / 2;
+  // the sticky status and the previous coefficients are only needed at the very end: load them now
+  const int status_in = D.status[s];
+  double xold = 0.0;
+  if (lane < nt) xold = D.X[(size_t)s * nt + lane];
   double A[NA], g[NT];
 #pragma unroll
   for (int k = 0; k < NA; ++k) A[k] = 0.0;
@@ -178,6 +182,9 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
   bool any = false;
   #pragma unroll
   for (int l = 0; l < nt; ++l) { sc[l] = sqrt(A[l * (l + 1) / 2 + l]); any |= sc[l] > 0.0; }
+  double isc[NT];                              // reciprocal scales: one division per column instead of one per entry
+  #pragma unroll
+  for (int l = 0; l < nt; ++l) isc[l] = sc[l] > 0.0 ? 1.0 / sc[l] : 0.0;
   if (!finite) st = 2; else if (!any) st = 3;
   const double reg = D.lambda_reg * D.lambda_reg * (double)D.M;
   // scaled matrix (unit diagonal + reg); dropped columns (sc = 0) become identity rows
@@ -187,14 +194,17 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
     for (int l = 0; l < nt; ++l)
       #pragma unroll
       for (int q = 0; q <= l; ++q, ++k) {
-        if (sc[l] > 0.0 && sc[q] > 0.0) A[k] = A[k] / (sc[l] * sc[q]) + (l == q ? reg : 0.0);
+        if (sc[l] > 0.0 && sc[q] > 0.0) A[k] = A[k] * (isc[l] * isc[q]) + (l == q ? reg : 0.0);
         else A[k] = (l == q) ? 1.0 : 0.0;
       }
     #pragma unroll
-    for (int l = 0; l < nt; ++l) g[l] = sc[l] > 0.0 ? g[l] / sc[l] : 0.0;
+    for (int l = 0; l < nt; ++l) g[l] = g[l] * isc[l];
   }
   // Cholesky A = L L^T in place (row-packed lower triangle)
   double first_piv = 0.0;
+  double idg[NT];                              // 1 / L_ll
+  #pragma unroll
+  for (int l = 0; l < nt; ++l) idg[l] = 0.0;
   #pragma unroll
   for (int l = 0; l < nt; ++l) {
     if (st != 0) break;
@@ -206,9 +216,10 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
       if (q == l) {
         if (l == 0) first_piv = v;
         if (!(v > 1e-13 * first_piv) || !(v > 0.0)) { st = 3; break; }
-        A[l * (l + 1) / 2 + l] = sqrt(v);
+        idg[l] = rsqrt(v);
+        A[l * (l + 1) / 2 + l] = v * idg[l];
       } else {
-        A[l * (l + 1) / 2 + q] = v / A[q * (q + 1) / 2 + q];
+        A[l * (l + 1) / 2 + q] = v * idg[q];
       }
     }
   }
@@ -220,17 +231,17 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
       double v = g[l];
       #pragma unroll
       for (int p = 0; p < l; ++p) v -= A[l * (l + 1) / 2 + p] * X[p];
-      X[l] = v / A[l * (l + 1) / 2 + l];
+      X[l] = v * idg[l];
     }
     #pragma unroll
     for (int l = nt - 1; l >= 0; --l) {      // L^T x = z
       double v = X[l];
       #pragma unroll
       for (int p = l + 1; p < nt; ++p) v -= A[p * (p + 1) / 2 + l] * X[p];
-      X[l] = v / A[l * (l + 1) / 2 + l];
+      X[l] = v * idg[l];
     }
     #pragma unroll
-    for (int l = 0; l < nt; ++l) X[l] = sc[l] > 0.0 ? X[l] / sc[l] : 0.0;
+    for (int l = 0; l < nt; ++l) X[l] = X[l] * isc[l];
   }
   // chi^2 over the measurement rows
   double c2 = 0.0;
@@ -242,11 +253,11 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
     c2 = fma(rsum, rsum, c2);
   }
   c2 = warp_sum(c2);
-  if (lane == 0) {
-    const bool dead = D.status[s] != 0;       // status is sticky: a failed slice keeps its outputs
-    if (!dead) {
+  if (status_in == 0) {                        // status is sticky: a failed slice keeps its outputs
+    if (lane < nt) D.Xprev[(size_t)s * nt + lane] = xold;
+    if (lane == 0) {
       #pragma unroll
-      for (int l = 0; l < nt; ++l) { D.Xprev[(size_t)s * nt + l] = D.X[(size_t)s * nt + l]; D.X[(size_t)s * nt + l] = X[l]; }
+      for (int l = 0; l < nt; ++l) D.X[(size_t)s * nt + l] = X[l];
       D.chi2[s] = c2;
       if (st != 0) D.status[s] = st;
     }
