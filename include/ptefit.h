@@ -43,7 +43,7 @@ typedef struct { int nr, nz; double rmin, rmax, zmin, zmax; } ptefit_grid;
 /* Geometry.  All pointers are HOST memory, read during ptefit_create only. */
 typedef struct {
   int n_meas;                     /* M: magnetic probes + flux loops (rows of Eq. 2)            */
-  int n_coil;                     /* n_c: PF coils + eddy filaments (columns of G_C)            */
+  int n_coil;                     /* n_c: PF coils + eddy filaments (columns of G_C), <= 768     */
   const double *sigma;            /* [n_meas] 1-sigma of each channel, > 0 (fit weights 1/sigma)*/
   int n_lim;                      /* limiter polygon vertices, 1..256            */
   const double *lim_r, *lim_z;    /* [n_lim] inside the grid rectangle                          */

@@ -180,6 +180,16 @@ def _design_job(k):
                    xpt=np.array(d["xpt"][:4], float), axis=np.array(d["axis"][:4], float), ip=float(d["I"].sum()), max_pf=d["max_pf"])
 
 
+def _design_until_ok(seed):
+    nfail = 0
+    while True:
+        _, d = _design_job(seed)
+        if d is not None:
+            return seed, d, nfail
+        seed += 10000
+        nfail += 1
+
+
 def _accept_job(args):
     k, b, ic, sigma = args
     dev = _W["dev"]
@@ -239,20 +249,17 @@ def generate(cfg, jobs):
                     stats[s] = (rate, chi2, lim)
                 else:
                     rejected.append((s, out[s][0], f"accept status={st} rate={rate:.2f} limited={lim}"))
-                    seed = out[s][0] + 10000
-                    while True:
-                        _, d = ex.submit(_design_job, seed).result()
-                        if d is not None:
-                            break
-                        rejected.append((s, seed, "design"))
-                        seed += 10000
-                    out[s] = (seed, d)
-                    b[s] = noisy(s, seed, d)
                     redo.append(s)
+            # replacement seeds for the rejected slots, designed in parallel (a worker keeps trying seed + 10000 k)
+            new = list(ex.map(_design_until_ok, [out[s][0] + 10000 for s in redo], chunksize=1))
+            for s, (seed, d, nfail) in zip(redo, new):
+                rejected.extend((s, seed - 10000 * (k + 1), "design") for k in range(nfail))
+                out[s] = (seed, d)
+                b[s] = noisy(s, seed, d)
             todo = redo
     os.makedirs(CASE_DIR, exist_ok=True)
     M = c["n_probe"] + c["n_loop"]
-    nb = c["n_p"] + c["n_ff"]
+    nb = c["n_p"] + c["n_ff"] + (5 if c.get("spline") else 0)
     np.savez_compressed(
         os.path.join(CASE_DIR, cfg + ".npz"),
         b=np.stack([b[s] for s in range(n)]), ic=np.stack([out[s][1]["ic"] for s in range(n)]), sigma=sigma,

@@ -7,38 +7,56 @@
 namespace ptefit {
 
 // A0 / A0': d = b - G_C I_C (Eq. 2/6) and psi_coil = G_GC I_C; resets state.
-// grid (ceil(N/256), B), block 256.
+// Each block handles SETUP_S slices of 256 nodes, so that a table value read once feeds SETUP_S products
+// (the coil -> grid table is re-read from L2 for every slice otherwise).
+// grid (ceil(N/256), ceil(B/SETUP_S)), block 256, dyn smem SETUP_S * nc * sizeof(T).
+constexpr int SETUP_S = 8;
 template <typename T>
-__global__ void k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__ ic) {
+__global__ void __launch_bounds__(256) k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__ ic, int B) {
   extern __shared__ unsigned char smem_raw[];
-  T *sic = reinterpret_cast<T *>(smem_raw);
-  const int s = blockIdx.y;
+  T *sic = reinterpret_cast<T *>(smem_raw);                 // [SETUP_S][nc]
+  const int s0 = blockIdx.y * SETUP_S, ns = min(SETUP_S, B - s0);
   if (!b) { b = reinterpret_cast<const T *>(D.ca->b); ic = reinterpret_cast<const T *>(D.ca->ic); }   // graph replay: caller pointers from the argument block
-  for (int c = threadIdx.x; c < D.nc; c += blockDim.x) sic[c] = ic[(size_t)s * D.nc + c];
+  for (int e = threadIdx.x; e < SETUP_S * D.nc; e += blockDim.x) {
+    const int q = e / D.nc, c = e - q * D.nc;
+    sic[e] = q < ns ? ic[(size_t)(s0 + q) * D.nc + c] : T(0);
+  }
   __syncthreads();
   const int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n < D.N) {
     const T *g = D.ggc_t + n;                       // transposed table [n_c][N]: coalesced over nodes
-    T acc = T(0);
-#pragma unroll 4
-    for (int c = 0; c < D.nc; ++c) acc = fma(g[(size_t)c * D.N], sic[c], acc);
-    D.psi_coil[(size_t)s * D.N + n] = acc;
-  }
-  for (int m = n; m < D.M; m += gridDim.x * blockDim.x) {       // M may exceed the node count of a small grid
-    // FP64 accumulation: b and G_C I_C nearly cancel when the coil signal dominates the plasma signal, and an
-    // FP32 sum of n_c terms would leave d with a relative error of ~1e-6 |G_C I_C| / |d|
-    const T *g = D.gc + (size_t)m * D.nc;
-    double acc = 0.0;
-    for (int c = 0; c < D.nc; ++c) acc = fma((double)g[c], (double)sic[c], acc);
-    D.dred[(size_t)s * D.M + m] = D.fit_coils ? b[(size_t)s * D.M + m] : T((double)b[(size_t)s * D.M + m] - acc);   // Eq. 7 fits b itself
-  }
-  if (D.fit_coils)
-    for (int c = n; c < D.nc; c += gridDim.x * blockDim.x) {
-      const double v = (double)ic[(size_t)s * D.nc + c];
-      D.icm[(size_t)s * D.nc + c] = v; D.icf[(size_t)s * D.nc + c] = v;
+    T acc[SETUP_S];
+#pragma unroll
+    for (int q = 0; q < SETUP_S; ++q) acc[q] = T(0);
+#pragma unroll 2
+    for (int c = 0; c < D.nc; ++c) {
+      const T gv = g[(size_t)c * D.N];
+#pragma unroll
+      for (int q = 0; q < SETUP_S; ++q) acc[q] = fma(gv, sic[q * D.nc + c], acc[q]);
     }
-  if (n < D.nt) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
-  if (n == 0) { D.status[s] = 0; D.chi2[s] = 0.0; }
+#pragma unroll
+    for (int q = 0; q < SETUP_S; ++q)
+      if (q < ns) D.psi_coil[(size_t)(s0 + q) * D.N + n] = acc[q];
+  }
+  for (int q = 0; q < ns; ++q) {
+    const int s = s0 + q;
+    const T *sq = sic + q * D.nc;
+    for (int m = n; m < D.M; m += gridDim.x * blockDim.x) {       // M may exceed the node count of a small grid
+      // FP64 accumulation: b and G_C I_C nearly cancel when the coil signal dominates the plasma signal, and an
+      // FP32 sum of n_c terms would leave d with a relative error of ~1e-6 |G_C I_C| / |d|
+      const T *g = D.gc + (size_t)m * D.nc;
+      double acc = 0.0;
+      for (int c = 0; c < D.nc; ++c) acc = fma((double)g[c], (double)sq[c], acc);
+      D.dred[(size_t)s * D.M + m] = D.fit_coils ? b[(size_t)s * D.M + m] : T((double)b[(size_t)s * D.M + m] - acc);   // Eq. 7 fits b itself
+    }
+    if (D.fit_coils)
+      for (int c = n; c < D.nc; c += gridDim.x * blockDim.x) {
+        const double v = (double)ic[(size_t)s * D.nc + c];
+        D.icm[(size_t)s * D.nc + c] = v; D.icf[(size_t)s * D.nc + c] = v;
+      }
+    if (n < D.nt) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
+    if (n == 0) { D.status[s] = 0; D.chi2[s] = 0.0; }
+  }
 }
 
 // O2 cold start (paper silent): xn = ((R-Rc)/a)^2 + ((Z-Zc)/b)^2 where < 1 and

@@ -379,7 +379,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   if (g->nz < 9 || g->nz > 257 || (p2 & (p2 - 1)) != 0) return fail(h, PTEFIT_ERR_INVALID_ARG, "nz-1 must be a power of two in [8,256]");
   if (g->nr < 5 || g->nr > 257) return fail(h, PTEFIT_ERR_INVALID_ARG, "nr must be in [5,257]");
   if (!(g->rmin > 0.0) || !(g->rmax > g->rmin) || !(g->zmax > g->zmin)) return fail(h, PTEFIT_ERR_INVALID_ARG, "bad grid extents");
-  if (ge->n_meas < 1 || ge->n_coil < 1 || ge->n_coil > 1024 || !ge->sigma || !ge->lim_mask || !ge->lim_r || !ge->lim_z)
+  if (ge->n_meas < 1 || ge->n_coil < 1 || ge->n_coil > 768 || !ge->sigma || !ge->lim_mask || !ge->lim_r || !ge->lim_z)
     return fail(h, PTEFIT_ERR_INVALID_ARG, "bad geometry");
   if (ge->n_lim < 1 || ge->n_lim > PTEFIT_MAX_LIM) return fail(h, PTEFIT_ERR_INVALID_ARG, "n_lim must be in [1,256]");
   if (ge->ip_sign != 1 && ge->ip_sign != -1) return fail(h, PTEFIT_ERR_INVALID_ARG, "ip_sign must be +-1");
@@ -419,7 +419,7 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   }
   if (ba->lsq_method != 0 && ba->lsq_method != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "lsq_method must be 0 (normal equations) or 1 (Gram-Schmidt QR)");
   if (ba->fit_coils != 0 && ba->fit_coils != 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "fit_coils must be 0 or 1");
-  if (ba->lsq_method == 1) {
+  if (ba->lsq_method == 1 || ba->n_terms > 12) {
     const size_t sm = ((size_t)(ge->n_meas + ba->n_terms) * (ba->n_terms + 1) + (size_t)ba->n_terms * (ba->n_terms + 1) + ba->n_terms) * sizeof(double);
     if (sm > 48 * 1024) return fail(h, PTEFIT_ERR_UNSUPPORTED, "lsq_method 1: (n_meas + n_terms)(n_terms + 1) doubles must fit 48 KB of shared memory");
   }
@@ -434,6 +434,8 @@ extern "C" ptefit_status ptefit_create(const ptefit_grid *g, const ptefit_geomet
   if (op->gemm != PTEFIT_GEMM_3XTF32 && op->gemm != PTEFIT_GEMM_FFMA) return fail(h, PTEFIT_ERR_INVALID_ARG, "gemm must be PTEFIT_GEMM_3XTF32 or PTEFIT_GEMM_FFMA");
   if (op->flags & ~(PTEFIT_OPT_NO_GRAPH | PTEFIT_OPT_NO_FUSED_BASIS | PTEFIT_OPT_SOLVE_FFMA)) return fail(h, PTEFIT_ERR_INVALID_ARG, "unknown option flag");
   if (op->tc_split_k < 0) return fail(h, PTEFIT_ERR_INVALID_ARG, "tc_split_k must be >= 0");
+  if (op->gemm == PTEFIT_GEMM_FFMA && ba->n_terms > 12) return fail(h, PTEFIT_ERR_UNSUPPORTED, "PTEFIT_GEMM_FFMA supports at most 12 terms");
+  if (ba->fit_coils && ba->n_terms > 12) return fail(h, PTEFIT_ERR_UNSUPPORTED, "fit_coils supports at most 12 terms");
   if (ba->n_terms == 1 && ba->terms[0].kind == 2) return fail(h, PTEFIT_ERR_INVALID_ARG, "need at least one P'/FF' term");
   if (!(ba->lambda_reg >= 0.0) || !(ba->relax > 0.0) || ba->relax > 1.0) return fail(h, PTEFIT_ERR_INVALID_ARG, "need lambda_reg >= 0 and 0 < relax <= 1");
   if (op->max_batch < 1 || op->max_batch > 65535) return fail(h, PTEFIT_ERR_INVALID_ARG, "max_batch must be in [1,65535]");

@@ -287,8 +287,11 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
           if (l < NP) v = in[t] ? (pwv[t][l] - pwv[t][NP]) * r[t] : 0.f;
           else if (l < NPOLY) v = in[t] ? (pwv[t][l - NP] - pwv[t][NFF]) * f[t] : 0.f;
           else v = d[t];
-          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(hr[t]) : "f"(v));
-          asm("cvt.rna.tf32.f32 %0, %1;\n" : "=r"(lr[t]) : "f"(v - __uint_as_float(hr[t])));
+          // hi = v rounded to TF32 (add half an ulp of the 10-bit mantissa, clear the low 13 bits: two
+          // instructions where cvt.rna.tf32.f32 costs four on sm_100a); lo = v - hi exactly, its low bits
+          // are ignored by the tensor core
+          hr[t] = (__float_as_uint(v) + 0x1000u) & 0xffffe000u;
+          lr[t] = __float_as_uint(v - __uint_as_float(hr[t]));
         }
         const uint32_t off = rowbase + (uint32_t)l * 128u + (((uint32_t)kq ^ (uint32_t)l) << 4);
         *reinterpret_cast<uint4 *>(ahi + off) = make_uint4(hr[0], hr[1], hr[2], hr[3]);

@@ -19,7 +19,7 @@ CONFIGS = {
     "cfg4": dict(idx=4, n=129, zmax=1.6, n_probe=100, n_loop=40, n_pf=16, n_eddy=60, n_p=3, n_ff=3,
                  batch=512, n_iter=20, precision="fp32", ic_range=30e3,
                  shapes=("limited", "limited", "lsn", "usn", "dn")),   # 40/20/20/20 %
-    "cfg5": dict(idx=5, n=257, zmax=1.6, n_probe=100, n_loop=40, n_pf=16, n_eddy=60, n_p=4, n_ff=4,
+    "cfg5": dict(idx=5, n=257, zmax=1.6, n_probe=100, n_loop=40, n_pf=16, n_eddy=60, n_p=4, n_ff=4, spline=True,
                  batch=64, n_iter=30, precision="fp64", ic_range=30e3,
                  shapes=("limited", "limited", "lsn", "usn", "dn")),
 }
@@ -132,8 +132,12 @@ def make_device(name, with_tables=True):
                 cold_rc=0.80, cold_zc=0.0, cold_a=0.40, cold_b=0.72)
     meta = dict(cfg=c, name=name, r=r, z=z, sen_r=sen_r, sen_z=sen_z, alpha=alpha, n_probe=c["n_probe"],
                 src_r=src_r, src_z=src_z, src_w=src_w, n_pf=c["n_pf"])
-    out = dict(grid=grid, geom=geom, basis=dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=LAMBDA_REG, delz=1, relax=RELAX),
-               meta=meta, tables=None)
+    basis = dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=LAMBDA_REG, delz=1, relax=RELAX)
+    if c.get("spline"):
+        # BASELINE.json configs[4]: "plus 5-knot tension-spline FF' edge terms" (7 knots
+        # 0.70 .. 1.00, tension 10, the five interior cardinal functions)
+        basis["spline"] = dict(knots=np.linspace(0.70, 1.00, 7), tension=10.0, terms=[1, 2, 3, 4, 5])
+    out = dict(grid=grid, geom=geom, basis=basis, meta=meta, tables=None)
     if with_tables:
         out["tables"] = make_tables(meta, grid)
     return out

@@ -71,7 +71,8 @@ def check_slice(out, q, ores, dev, precision, strict_index=True):
         return dict(psi=0.0, coef=0.0, index_ok=True)
     sr = ores["srch"]
     epsi = psi_rel_err(out["psi"][q], ores["psi"])
-    ecoef = coef_rel_err(out["coeffs"][q].astype(np.float64), ores["X"], b["n_p"], b["n_ff"], dz)
+    n_ffk = b["n_ff"] + (len(b["spline"]["terms"]) if b.get("spline") else 0)      # spline terms are FF'-type columns
+    ecoef = coef_rel_err(out["coeffs"][q].astype(np.float64), ores["X"], b["n_p"], n_ffk, dz)
     assert epsi <= PSI_TOL[precision], (q, "psi", epsi)
     assert ecoef <= COEF_TOL, (q, "coef", ecoef)
     npoly = len(ores["X"]) - int(b.get("delz", 0))

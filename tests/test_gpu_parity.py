@@ -194,15 +194,23 @@ def test_joint_coil_fit_eq7(name, precision, ns):
     rec.close()
 
 
-def test_cfg5_reduced_fp64():
-    """BASELINE config 5 grid (257x257, FP64, 76 coil columns, 4+4 terms), 2 slices, 30 iterations.
-    The tension-spline edge terms of config 5 are not implemented yet (DESIGN.md gaps)."""
-    dev, sl = cached_case("cfg5", 2)
+def test_cfg5_as_specified_fp64():
+    """BASELINE config 5 as stated: 257x257, FP64 on the FP64 tensor cores (k_gemm_dmma), 76 coil columns,
+    p' 4 terms + FF' 4 terms + 5 tension-spline FF' edge terms (+ delz) = 14 fitted terms, 30 iterations.
+    8 slices of the batch (limited, lower / upper single null, double null: the null shapes are diverted)
+    against the oracle at 1e-10."""
+    dev, sl = cached_case("cfg5", 8)
+    assert dev["basis"]["spline"] is not None and len(dev["basis"]["spline"]["terms"]) == 5
     od = oracle_device(dev)
-    rec, out = _run_gpu(dev, sl["b"], sl["ic"], 30, "fp64", max_batch=4)
-    for q in range(2):
+    rec, out = _run_gpu(dev, sl["b"], sl["ic"], 30, "fp64", max_batch=8)
+    assert rec.nt == 14
+    n_div = 0
+    for q in range(8):
         ores = reconstruct(od, sl["b"][q], sl["ic"][q], 30)
+        assert ores["status"] == 0
         check_slice(out, q, ores, dev, "fp64")
+        n_div += ores["srch"]["limited"] == 0
+    assert n_div >= 3                                   # lsn, usn, dn slices end diverted
     rec.close()
 
 
