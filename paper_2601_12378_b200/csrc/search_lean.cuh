@@ -42,6 +42,13 @@ struct LeanShared {
 #define LS_T(k) do { } while (0)
 #endif
 
+// Indices of the non-zero words of the static masks (host-built, copied to shared memory): the loops of the
+// search run over these lists, so every warp iteration does useful work and the words are dealt round-robin.
+struct WordLists {
+  const unsigned short *lim, *xpt, *dil, *zero;      // lim_mask words, xpt_mask words, dilated-by-one words, words with dil2 bits but no lim bit
+  int n_lim, n_xpt, n_dil, n_zero;
+};
+
 // FP32 pre-filter of one node: false = certainly not a candidate.  A candidate has its stationary
 // point (x*, y*) inside the half cell, and the fitted gradient at the node is -H (x*, y*), hence
 // |cx| <= |cxx| + |cxy|/2 and |cy| <= |cyy| + |cxy|/2.  Tested in FP32 with a 2 % margin plus an absolute
@@ -78,9 +85,8 @@ __device__ __noinline__ void xpt_decide(double rmin, double zmin, double dr, dou
 // memory, overwritten per lim_mask word with I'(xn) (pc != nullptr) or xn; xn: global, lim_mask words
 // only.  (am_v, am_n) / bad: this thread's partial arg-max of s psi over lim_mask and finiteness flag.
 __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, int s, float *psi, float *__restrict__ xn,
-                                            const unsigned *__restrict__ lbits, const unsigned *__restrict__ xbits, const unsigned *__restrict__ d2bits, float am_v,
-                                            int am_n,
-                                            bool bad, const float *pc, const float *rdA, const float *fdA, const double *Xs) {
+                                            const unsigned *__restrict__ lbits, const unsigned *__restrict__ xbits, const unsigned *__restrict__ d2bits,
+                                            const WordLists &WL, float am_v, int am_n, bool bad, const float *pc, const float *rdA, const float *fdA, const double *Xs) {
   const int nth = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
   const int nr = D.nr, N = D.N, nwords = (N + 31) >> 5;
   const double sg = (double)D.ip_sign;
@@ -123,11 +129,12 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
   }
   LS_T(0);
   // 2. X-point candidates: FP32 scan of the xpt_mask words -> compact list (the scan does not need the axis)
-  for (int w = warp; w < nwords; w += nwarp) {
-    const unsigned xw = xbits[w];
-    if (!xw) continue;
+#pragma unroll 2
+  for (int k = warp; k < WL.n_xpt; k += nwarp) {
+    const int w = WL.xpt[k];
     const int n = (w << 5) + lane;
-    if (((xw >> lane) & 1u) && xpt_prefilter(psi + n, nr)) {
+    const bool bit = (xbits[w] >> lane) & 1u;
+    if (xpt_prefilter(psi + (bit ? n : nr + 1), nr) && bit) {         // masked-off lanes read a harmless interior node
       const int q = atomicAdd(&S.nlist, 1);
       if (q < LEAN_LIST) S.list[q] = n;
     }
@@ -141,11 +148,10 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
     if (nl <= LEAN_LIST) {
       for (int q = tid; q < nl; q += nth) xpt_decide(D.rmin, D.zmin, D.dr, D.dz, nr, &S, psi, S.list[q], sg, Pa);
     } else {                                     // list overflow (not seen on smooth flux): decide in place
-      for (int w = warp; w < nwords; w += nwarp) {
-        const unsigned xw = xbits[w];
-        if (!xw) continue;
+      for (int k = warp; k < WL.n_xpt; k += nwarp) {
+        const int w = WL.xpt[k];
         const int n = (w << 5) + lane;
-        if (((xw >> lane) & 1u) && xpt_prefilter(psi + n, nr)) xpt_decide(D.rmin, D.zmin, D.dr, D.dz, nr, &S, psi, n, sg, Pa);
+        if (((xbits[w] >> lane) & 1u) && xpt_prefilter(psi + n, nr)) xpt_decide(D.rmin, D.zmin, D.dr, D.dz, nr, &S, psi, n, sg, Pa);
       }
     }
   }
@@ -243,67 +249,66 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
     float pp[5], pq[5];                               // low-degree fast path: coefficients in registers
 #pragma unroll
     for (int k = 0; k < 5; ++k) { pp[k] = pc ? pc[k] : 0.f; pq[k] = pc ? pc[MD + 1 + k] : 0.f; }
-    for (int w = warp; w < nwords; w += nwarp) {
-      const unsigned lw = lbits[w];
-      if (!lw) {                                      // rows the delz stencil reaches: I' = 0 there
-        if (pc && ((d2bits[w] >> lane) & 1u)) psi[(w << 5) + lane] = 0.f;
-        continue;
-      }
+    const bool spl = D.nspl && Xs;
+#pragma unroll 2
+    for (int k = warp; k < WL.n_lim; k += nwarp) {
+      const int w = WL.lim[k];
       const int n = (w << 5) + lane;
-      if (n >= N) continue;
-      float out = -1.f;
-      int i = 0;
-      if ((lw >> lane) & 1u) {
-        const int j = __float2int_rd(((float)n + 0.5f) * inv_nr);     // exact: (n + 0.5)/nr is >= 0.5/nr away from an integer
-        i = n - j * nr;
-        const float v = psi[n];
-        if (sgf * v > thr) {
-          bool in = true;
-          for (int c = 0; c < ncand; ++c) {
-            const float val = fmaf(S.hR[c], (float)i, fmaf(S.hZ[c], (float)j, S.h0[c]));
-            if (fabsf(val) > S.hm[c]) in &= val > 0.f;
-            else {
-              const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
-              in &= ((R - S.cR[c]) * (Ra - S.cR[c]) + (Z - S.cZ[c]) * (Za - S.cZ[c])) > 0.0;
-            }
+      const bool bit = (lbits[w] >> lane) & 1u;
+      const int j = __float2int_rd(((float)n + 0.5f) * inv_nr);     // exact: (n + 0.5)/nr is >= 0.5/nr away from an integer
+      const int i = n - j * nr;
+      const float v = psi[bit ? n : 0];
+      bool in = bit && (sgf * v > thr);
+      if (ncand) {                                    // uniform branch
+        for (int c = 0; c < ncand; ++c) {
+          const float val = fmaf(S.hR[c], (float)i, fmaf(S.hZ[c], (float)j, S.h0[c]));
+          bool ok = val > 0.f;
+          if (in && !(fabsf(val) > S.hm[c])) {        // inside the FP32 error margin: the FP64 expression decides (rare)
+            const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
+            ok = ((R - S.cR[c]) * (Ra - S.cR[c]) + (Z - S.cZ[c]) * (Za - S.cZ[c])) > 0.0;
           }
-          if (in) {
-            const float d = (v - pa_hi) - pa_lo;
-            out = fminf(fmaxf(fmaf(d, inv_lo, d * inv_hi), 0.f), 1.f);
-            ++cnt;
-          }
+          in = in && ok;
         }
       }
-      xn[n] = out;
+      const float d = (v - pa_hi) - pa_lo;
+      const float x = fminf(fmaxf(fmaf(d, inv_lo, d * inv_hi), 0.f), 1.f);
+      const float out = in ? x : -1.f;
+      cnt += in;
+      if (n < N) xn[n] = out;
       float lv = out;
-      if (pc) {                                       // I'(x) = rdA P(x) + fdA Q(x) by Horner (delz column)
-        lv = 0.f;
-        if (!(out < 0.f)) {
-          float hp, hq;
-          if (lowdeg) {
-            hp = pp[4]; hq = pq[4];
+      if (pc) {                                       // I'(x) = rdA P(x) + fdA Q(x) by Horner (delz column); uniform branch
+        float hp, hq;
+        if (lowdeg) {
+          hp = pp[4]; hq = pq[4];
 #pragma unroll
-            for (int k = 3; k >= 0; --k) { hp = fmaf(hp, out, pp[k]); hq = fmaf(hq, out, pq[k]); }
-          } else {
-            hp = pc[MD]; hq = pc[2 * MD + 1];
+          for (int q = 3; q >= 0; --q) { hp = fmaf(hp, x, pp[q]); hq = fmaf(hq, x, pq[q]); }
+        } else {
+          hp = pc[MD]; hq = pc[2 * MD + 1];
 #pragma unroll
-            for (int k = MD - 1; k >= 0; --k) { hp = fmaf(hp, out, pc[k]); hq = fmaf(hq, out, pc[MD + 1 + k]); }
-          }
-          lv = fmaf(rdA[i], hp, fdA[i] * hq);
-          if (D.nspl && Xs) lv += spline_current(D, Xs, out, rdA[i], fdA[i]);
+          for (int q = MD - 1; q >= 0; --q) { hp = fmaf(hp, x, pc[q]); hq = fmaf(hq, x, pc[MD + 1 + q]); }
         }
+        const int ic = min(i, nr - 1);
+        lv = fmaf(rdA[ic], hp, fdA[ic] * hq);
+        if (spl && in) lv += spline_current(D, Xs, x, rdA[ic], fdA[ic]);
+        lv = in ? lv : 0.f;
       }
-      psi[n] = lv;
+      if (n < N) psi[n] = lv;
     }
-  } else {
-    for (int w = warp; w < nwords; w += nwarp) {
-      const int n = (w << 5) + lane;
-      if (!lbits[w]) {
-        if (pc && ((d2bits[w] >> lane) & 1u)) psi[n] = 0.f;
-        continue;
+    if (pc)                                           // rows the delz stencil reaches beyond the lim_mask words: I' = 0 there
+      for (int k = warp; k < WL.n_zero; k += nwarp) {
+        const int w = WL.zero[k];
+        if ((d2bits[w] >> lane) & 1u) psi[(w << 5) + lane] = 0.f;
       }
+  } else {
+    for (int k = warp; k < WL.n_lim; k += nwarp) {
+      const int n = (WL.lim[k] << 5) + lane;
       if (n < N) { xn[n] = -1.f; psi[n] = pc ? 0.f : -1.f; }
     }
+    if (pc)
+      for (int k = warp; k < WL.n_zero; k += nwarp) {
+        const int w = WL.zero[k];
+        if ((d2bits[w] >> lane) & 1u) psi[(w << 5) + lane] = 0.f;
+      }
   }
   LS_T(5);
   cnt = __reduce_add_sync(0xffffffffu, cnt);

@@ -42,6 +42,8 @@ constexpr int TCS_OP_BYTES = 131072;        // operand tiles: 4 x [128][64] floa
 struct TcSolveDev {
   const double *tcib;         // [128][128] inverse pivots of the Thomas factorisation, [row i][TMEM lane]; rows >= nri are 1
   const double *tcw, *tce;    // [nri] sub- and super-diagonal of the tridiagonal systems (cw_i, ce_i)
+  const unsigned short *wl;   // [4][nwords] indices of the non-zero words of the lim / xpt / dilated / zero-only masks (WordLists)
+  int n_lim, n_xpt, n_dil, n_zero;
 };
 
 __host__ __device__ inline size_t tcs_smem_bytes(int nr, int nz) {
@@ -50,6 +52,7 @@ __host__ __device__ inline size_t tcs_smem_bytes(int nr, int nz) {
   b += 4 * nwords * sizeof(unsigned);                      // lim / xpt / dilated lim (1 and 2 rows) bit masks
   b += (size_t)(2 * (nr + nz)) * sizeof(float);            // boundary flux
   b += 2 * (size_t)nr * sizeof(double);                    // sub- and super-diagonal
+  b += 4 * nwords * sizeof(unsigned short) + 16;           // word lists of the search
   return b + 64;
 }
 
@@ -122,6 +125,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   T *pb = reinterpret_cast<T *>(mbits + 4 * nwords);       // bottom[nr], top[nr], left[nzi], right[nzi]
   double *ce_s = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(pb + 2 * (nr + nz)) + ((8u - (tc::smem_u32(pb + 2 * (nr + nz)) & 7u)) & 7u));
   double *cw_s = ce_s + nr;
+  unsigned short *wls = reinterpret_cast<unsigned short *>(cw_s + nr);   // [4][nwords]
   const double *ibs = reinterpret_cast<const double *>(op);   // Thomas phase: inverse pivots [i][lane], staged by bulk copies
   __shared__ uint64_t bar_tab, bar_mma, bar_ib[8];
   __shared__ uint32_t tmem_slot;
@@ -142,6 +146,10 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   if (warp == 0) tc::tmem_alloc<512>(&tmem_slot);
   for (int w = tid; w < 4 * nwords; w += nth)
     mbits[w] = (w < nwords) ? D.lim_bits[w] : (w < 2 * nwords) ? D.xpt_bits[w - nwords] : (w < 3 * nwords) ? D.dil_bits[w - 2 * nwords] : D.dil2_bits[w - 3 * nwords];
+  for (int w = tid; w < 4 * nwords; w += nth) wls[w] = S.wl[w];
+  WordLists WL;
+  WL.lim = wls; WL.xpt = wls + nwords; WL.dil = wls + 2 * nwords; WL.zero = wls + 3 * nwords;
+  WL.n_lim = S.n_lim; WL.n_xpt = S.n_xpt; WL.n_dil = S.n_dil; WL.n_zero = S.n_zero;
   for (int i = tid; i < nr; i += nth) {
     const double Rd = D.rmin + i * D.dr;
     c_rhs[i] = T(-kMu0 * Rd / D.dA);
@@ -454,7 +462,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
     TCS_T(4);
     if (do_search) {
       float *xn = xn_all + (size_t)s * N;
-      search_lean(D, lean, s, G, xn, mbits, mbits + nwords, mbits + 3 * nwords, am_v, am_n, bad0, D.has_delz ? pcoef : nullptr, c_rdA, c_fdA,
+      search_lean(D, lean, s, G, xn, mbits, mbits + nwords, mbits + 3 * nwords, WL, am_v, am_n, bad0, D.has_delz ? pcoef : nullptr, c_rdA, c_fdA,
                   D.X + (size_t)s * D.nt);                 // G now holds I'(xn) (delz) or xn on the lim_mask words
       TCS_T(5);
       if (D.has_delz) {
@@ -464,11 +472,11 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
         float *dzc = D.dzc + (size_t)s * N;
         const float hz = float(0.5 / D.dz);
         const unsigned *dbits = mbits + 2 * nwords;
-        for (int w = warp; w < nwords; w += nth >> 5) {
-          const unsigned dw = dbits[w];
-          if (!dw) continue;
+#pragma unroll 2
+        for (int k = warp; k < WL.n_dil; k += nth >> 5) {
+          const int w = WL.dil[k];
           const int n = (w << 5) + lane;
-          if ((dw >> lane) & 1u) dzc[n] = -(G[n + nr] - G[n - nr]) * hz;     // G = 0 off the lim_mask nodes (search_lean)
+          if ((dbits[w] >> lane) & 1u) dzc[n] = -(G[n + nr] - G[n - nr]) * hz;     // G = 0 off the lim_mask nodes (search_lean)
         }
       }
       TCS_T(6);
