@@ -554,3 +554,63 @@ def test_large_batch_beyond_one_wave_of_row_tiles():
     for q in range(8, B):
         assert np.array_equal(out["psi"][q], out["psi"][q % 8]) and np.array_equal(out["coeffs"][q], out["coeffs"][q % 8]), q
     rec.close()
+
+
+@pytest.mark.parametrize("name,precision", [("cfg1", "fp64"), ("cfg3", "fp32")])
+def test_negative_plasma_current_mirror(name, precision):
+    """ip_sign = -1: with every measurement and coil current negated the reconstruction is the exact mirror
+    image (psi -> -psi, coefficients -> -X, same axis / X-point nodes, same chi2) -- the mirror pin SURVEY.md
+    8(c) lists for the search rules, here through the whole CUDA path -- and matches the oracle run with s = -1."""
+    torch = _torch()
+    dev, sl = cached_case(name, 2)
+    dv, b, ic = round_inputs(dev, sl, precision)
+    n_iter = dev["meta"]["cfg"]["n_iter"]
+    rec, out = _run_gpu(dev, b, ic, n_iter, precision)
+    dn = dict(dev); dn["geom"] = dict(dev["geom"], ip_sign=-1)
+    recn, outn = _run_gpu(dn, -b, -ic, n_iter, precision)
+    for q in range(2):
+        assert int(outn["status"][q]) == int(out["status"][q]) == 0
+        assert np.array_equal(outn["psi"][q], -out["psi"][q])
+        assert np.array_equal(outn["axis_ij"][q], out["axis_ij"][q]) and np.array_equal(outn["xpt_ij"][q], out["xpt_ij"][q])
+        assert int(outn["limited"][q]) == int(out["limited"][q])
+        assert np.array_equal(outn["coeffs"][q][:-1], -out["coeffs"][q][:-1]) and outn["coeffs"][q][-1] == out["coeffs"][q][-1]
+        assert outn["psi_bnd"][q] == -out["psi_bnd"][q] and outn["chi2"][q] == out["chi2"][q]
+    dvn = dict(dv); dvn["geom"] = dict(dv["geom"], ip_sign=-1)
+    odn = oracle_device(dvn)
+    ores = reconstruct(odn, -b[0], -ic[0], n_iter)
+    check_slice(outn, 0, ores, dn, precision, strict_index=(precision == "fp64"))
+    rec.close(); recn.close()
+
+
+def test_warm_start_and_ragged_batch_fp32_tc_path():
+    """FP32 tensor-core path (k_solve_tc, in-GEMM basis producer): a batch of 3 inside a max_batch = 5 handle,
+    8 iterations from the cold start, then 4 more from the returned flux (k_search start), against the oracle
+    continued the same way; then the paper's mode, one warm iteration at a time, four times."""
+    torch = _torch()
+    dev, sl = cached_case("cfg3", 3)
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    od = oracle_device(dv)
+    rec = _rec(dev, "fp32", 5)
+    db = torch.tensor(b, dtype=rec.dtype, device="cuda"); dic = torch.tensor(ic, dtype=rec.dtype, device="cuda")
+    rec.reconstruct(db, dic, 8)
+    rec.reconstruct(db, dic, 4, warm_start=True)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, 3)
+    o12 = []
+    for q in range(3):
+        o8 = reconstruct(od, b[q], ic[q], 8)
+        ow = reconstruct(od, b[q], ic[q], 4, psi0=o8["psi"])
+        o12.append(ow)
+        assert ow["status"] == 0 and int(out["status"][q]) == 0
+        assert psi_rel_err(out["psi"][q], ow["psi"]) <= PSI_TOL["fp32"], q
+        assert tuple(out["axis_ij"][q]) == tuple(ow["srch"]["axis"][:2])
+    for _ in range(4):
+        rec.reconstruct(db, dic, 1, warm_start=True)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, 3)
+    for q in range(3):
+        o = o12[q]
+        for _ in range(4):
+            o = reconstruct(od, b[q], ic[q], 1, psi0=o["psi"])
+        assert psi_rel_err(out["psi"][q], o["psi"]) <= PSI_TOL["fp32"], q
+    rec.close()
