@@ -88,7 +88,7 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
                                             const unsigned *__restrict__ lbits, const unsigned *__restrict__ xbits, const unsigned *__restrict__ d2bits,
                                             const WordLists &WL, float am_v, int am_n, bool bad, const float *pc, const float *rdA, const float *fdA, const double *Xs) {
   const int nth = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nwarp = nth >> 5;
-  const int nr = D.nr, N = D.N, nwords = (N + 31) >> 5;
+  const int nr = D.nr, N = D.N;
   const double sg = (double)D.ip_sign;
   if (tid == 0) { S.flag = 0; S.ncand = 0; S.count = 0; S.nlist = 0; }
 #ifdef PTEFIT_TUNING

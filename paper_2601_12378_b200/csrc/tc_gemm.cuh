@@ -137,7 +137,8 @@ struct AProd {
   int epi, RS, nri, nzi, nr;
   float scale;
 };
-template <int NP> constexpr int gemm_threads() { return NP > 0 ? 448 : GEMM_THREADS; }
+constexpr int PROD_GROUPS = 2;   // groups of four basis-producer warps; group g fills the K blocks kb0 + g, kb0 + g + PROD_GROUPS, ...
+template <int NP> constexpr int gemm_threads() { return NP > 0 ? GEMM_THREADS + 128 * PROD_GROUPS : GEMM_THREADS; }
 
 template <int BN, int STAGES, int NP = 0, int NFF = 0>
 __global__ void __launch_bounds__(gemm_threads<NP>(), 1)
@@ -227,13 +228,13 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         tc_commit(tfull + buf);                        // chunk complete
       }
     }
-  } else if (NP > 0 && warp >= 10) {                   // ---- basis producers (warps 10-13)
+  } else if (NP > 0 && warp >= 10) {                   // ---- basis producers (warps 10-17: two groups of four)
     constexpr int NPOLY = NP + NFF;
     constexpr int PMAX = NP > NFF ? NP : NFF;
     // lane -> (slice sq = lane >> 3 of the warp's four, node quad kq = lane & 7 of the block's
     // 32 nodes): four consecutive nodes of one slice per thread, so that every term row is one
     // 16-byte store per hi / lo tile (a quarter warp covers one 128-byte row: conflict free).
-    const int pw_ = warp - 10, sq = lane >> 3, kq = lane & 7;
+    const int pg = (warp - 10) >> 2, pw_ = (warp - 10) & 3, sq = lane >> 3, kq = lane & 7;
     const int sl = min(m0 / 8 + 4 * pw_ + sq, ap.B - 1);
     const float *xs = ap.xn + (size_t)sl * ap.N, *ds = ap.dzc + (size_t)sl * ap.N;
     // software pipeline of the gather: node indices and factors of block kb + 3, flux values of
@@ -272,8 +273,8 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
         for (int k = 1; k <= PMAX; ++k) pwv[t][k] = pwv[t][k - 1] * xb[t];
         in[t] = !(xb[t] < 0.f);
       }
-      fetch_val(kb + 2, xb, db, rb, fb);
-      fetch_idx(kb + 3);
+      fetch_val(kb + 2 * PROD_GROUPS, xb, db, rb, fb);
+      fetch_idx(kb + 3 * PROD_GROUPS);
       mbar_wait(empty + s, ph ^ 1u);
       unsigned char *ahi = base + s * L::STAGE_BYTES, *alo = ahi + L::A_BYTES;
       const uint32_t rowbase = (uint32_t)(4 * pw_ + sq) * 1024u;
@@ -303,14 +304,15 @@ k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapAhi, const __grid_constant_
     };
     float xa[4], da[4], xb2[4], db2[4];
     float4 ra, fa, rb2, fb2;
-    fetch_idx(kb0);
-    fetch_val(kb0, xa, da, ra, fa);
-    fetch_idx(kb0 + 1);
-    fetch_val(kb0 + 1, xb2, db2, rb2, fb2);
-    fetch_idx(kb0 + 2);
-    for (int kb = kb0, it = 0; kb < kb1; kb += 2, it += 2) {
-      step(kb, it, xa, da, ra, fa);
-      if (kb + 1 < kb1) step(kb + 1, it + 1, xb2, db2, rb2, fb2);
+    const int k0 = kb0 + pg;                             // this group's first K block
+    fetch_idx(k0);
+    fetch_val(k0, xa, da, ra, fa);
+    fetch_idx(k0 + PROD_GROUPS);
+    fetch_val(k0 + PROD_GROUPS, xb2, db2, rb2, fb2);
+    fetch_idx(k0 + 2 * PROD_GROUPS);
+    for (int kb = k0; kb < kb1; kb += 2 * PROD_GROUPS) {
+      step(kb, kb - kb0, xa, da, ra, fa);
+      if (kb + PROD_GROUPS < kb1) step(kb + PROD_GROUPS, kb + PROD_GROUPS - kb0, xb2, db2, rb2, fb2);
     }
   } else if (warp >= 2 && warp < 10) {                 // ---- promotion to registers + epilogue
     const int q = warp & 3;                            // TMEM lane quarter this warp may access
