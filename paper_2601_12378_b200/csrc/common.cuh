@@ -123,6 +123,29 @@ __device__ __forceinline__ double spline_phi(const SplineDev &sp, int q, double 
   return v;
 }
 
+// The pieces of spline_phi that do not depend on q: interval r, t, and the two sinh brackets (one pair of
+// sinh per node instead of one per spline term).
+struct SplinePt { int r; double t, A, Bc; bool in; };
+__device__ __forceinline__ SplinePt spline_point(const SplineDev &sp, double x) {
+  SplinePt p;
+  p.in = (x >= sp.knot[0]) && (x <= sp.knot[sp.nk - 1]);
+  int r = 0;
+  while (r < sp.nk - 2 && x >= sp.knot[r + 1]) ++r;
+  p.r = r;
+  p.t = fmin(fmax((x - sp.knot[r]) * sp.inv_h[r], 0.0), 1.0);
+  const double th = sp.tau_h[r];
+  p.A = sinh(th * (1.0 - p.t)) * sp.inv_sinh[r] - (1.0 - p.t);
+  p.Bc = sinh(th * p.t) * sp.inv_sinh[r] - p.t;
+  return p;
+}
+__device__ __forceinline__ double spline_phi_at(const SplineDev &sp, const SplinePt &p, int q) {
+  if (!p.in) return 0.0;
+  double v = (sp.m[p.r][q] * p.A + sp.m[p.r + 1][q] * p.Bc) * sp.inv_tau2;
+  if (q == p.r) v += 1.0 - p.t;
+  if (q == p.r + 1) v += p.t;
+  return v;
+}
+
 template <typename T>
 __device__ __forceinline__ T basis_term(const Dev<T> &D, int l, T x, T rdA, T mu0dA_over_r) {
   const TermDev t = D.terms[l];

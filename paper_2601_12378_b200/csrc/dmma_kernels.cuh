@@ -32,8 +32,13 @@ __global__ void __launch_bounds__(128) k_basis_c(Dev<double> D, DmDev Dm) {
   const int i = n % D.nr;
   const double R = D.rmin + i * D.dr;
   const double rdA = R * D.dA, fdA = kMu0 * D.dA / R;
+  SplinePt sp{};
+  if (D.nspl && x >= 0.0) sp = spline_point(*D.spl, x);
   for (int l = 0; l < D.nt; ++l) {
-    const double v = (l < D.npoly) ? basis_term(D, l, x, rdA, fdA) : D.dzc[(size_t)s * D.N + n];
+    double v;
+    if (l >= D.npoly) v = D.dzc[(size_t)s * D.N + n];
+    else if (D.terms[l].family == 1) v = x < 0.0 ? 0.0 : spline_phi_at(*D.spl, sp, D.terms[l].i) * (D.terms[l].kind == 0 ? rdA : fdA);
+    else v = basis_term(D, l, x, rdA, fdA);
     Dm.jb[((size_t)s * D.nt + l) * Dm.Kc + kc] = v;
   }
 }
