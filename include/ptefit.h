@@ -129,7 +129,9 @@ ptefit_status ptefit_create(const ptefit_grid *grid, const ptefit_geometry *geom
 ptefit_status ptefit_reconstruct(ptefit_handle *h, int batch,
     const void *d_b,        /* [batch][n_meas]  real: measurements b (Eq. 2)                    */
     const void *d_ic,       /* [batch][n_coil]  real: coil + eddy currents I_C                  */
-    int n_iter, int warm_start, /* warm_start = 1: d_psi holds the starting flux                */
+    int n_iter, int warm_start, /* warm_start = 1: d_psi holds the starting flux, and the coefficients
+                                   of this handle's previous call seed the vertical-shift column of the
+                                   first iteration (slice q continues slice q of that call)         */
     void *d_psi,            /* [batch][nz][nr]  real, in/out: poloidal flux per radian          */
     void *d_coeffs,         /* [batch][n_terms] real: X of the last fit (Eq. 11)                */
     int *d_axis_ij,         /* [batch][2] (i, j) of the axis node                               */

@@ -82,11 +82,14 @@ def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None, b
     return out
 
 
-def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False):
-    """ptefit_reconstruct for one slice.  psi0 = None -> cold start (O2), else warm start."""
+def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False, X0=None):
+    """ptefit_reconstruct for one slice.  psi0 = None -> cold start (O2), else warm start; X0 = the
+    coefficients of the previous call (a warm start keeps them: they seed the vertical-shift column of the
+    first iteration, which is what keeps the one-iteration-per-slice mode of PAPER.md:158 from drifting)."""
     d = np.asarray(b, np.float64) - dev.gc @ np.asarray(ic, np.float64)           # Eq. 2 / Eq. 6 rhs
     psi_coil = (dev.ggc @ np.asarray(ic, np.float64)).reshape(dev.nz, dev.nr)
-    res = dict(status=0, X=np.zeros(dev.nb), chi2=np.nan, psi=None, srch=None, hist=[])
+    res = dict(status=0, X=np.zeros(dev.nb) if (X0 is None or psi0 is None) else np.array(X0, np.float64), chi2=np.nan, psi=None,
+               srch=None, hist=[])
     if psi0 is None:
         psin, mask = _search.cold_start(dev.r, dev.z, dev.lim_mask, *dev.cold)
         psi = np.zeros((dev.nz, dev.nr))

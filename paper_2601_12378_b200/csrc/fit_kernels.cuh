@@ -6,13 +6,13 @@
 
 namespace ptefit {
 
-// A0 / A0': d = b - G_C I_C (Eq. 2/6) and psi_coil = G_GC I_C; resets state.
+// A0 / A0': d = b - G_C I_C (Eq. 2/6) and psi_coil = G_GC I_C; resets state (keep_x: not the coefficients).
 // Each block handles SETUP_S slices of 256 nodes, so that a table value read once feeds SETUP_S products
 // (the coil -> grid table is re-read from L2 for every slice otherwise).
 // grid (ceil(N/256), ceil(B/SETUP_S)), block 256, dyn smem SETUP_S * nc * sizeof(T).
 constexpr int SETUP_S = 8;
 template <typename T>
-__global__ void __launch_bounds__(256) k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__ ic, int B) {
+__global__ void __launch_bounds__(256) k_setup(Dev<T> D, const T *__restrict__ b, const T *__restrict__ ic, int B, int keep_x) {
   extern __shared__ unsigned char smem_raw[];
   T *sic = reinterpret_cast<T *>(smem_raw);                 // [SETUP_S][nc]
   const int s0 = blockIdx.y * SETUP_S, ns = min(SETUP_S, B - s0);
@@ -54,7 +54,8 @@ __global__ void __launch_bounds__(256) k_setup(Dev<T> D, const T *__restrict__ b
         const double v = (double)ic[(size_t)s * D.nc + c];
         D.icm[(size_t)s * D.nc + c] = v; D.icf[(size_t)s * D.nc + c] = v;
       }
-    if (n < D.nt) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
+    // a warm start keeps the coefficients of the handle's previous call: they seed the vertical-shift column
+    if (n < D.nt && !keep_x) { D.X[(size_t)s * D.nt + n] = 0.0; D.Xprev[(size_t)s * D.nt + n] = 0.0; }
     if (n == 0) { D.status[s] = 0; D.chi2[s] = 0.0; }
   }
 }

@@ -233,7 +233,7 @@ def test_edge_cases():
     torch.cuda.synchronize()
     out2 = _gpu_out(rec, 3)
     for q in range(3):
-        ow = reconstruct(od, b[q], ic[q], 2, psi0=o6[q]["psi"])
+        ow = reconstruct(od, b[q], ic[q], 2, psi0=o6[q]["psi"], X0=o6[q]["X"])
         assert psi_rel_err(out2["psi"][q], ow["psi"]) <= 1e-10
     # garbage input: all-zero measurements and currents -> the oracle's failure status
     z = torch.zeros_like(db)
@@ -599,7 +599,7 @@ def test_warm_start_and_ragged_batch_fp32_tc_path():
     o12 = []
     for q in range(3):
         o8 = reconstruct(od, b[q], ic[q], 8)
-        ow = reconstruct(od, b[q], ic[q], 4, psi0=o8["psi"])
+        ow = reconstruct(od, b[q], ic[q], 4, psi0=o8["psi"], X0=o8["X"])
         o12.append(ow)
         assert ow["status"] == 0 and int(out["status"][q]) == 0
         assert psi_rel_err(out["psi"][q], ow["psi"]) <= PSI_TOL["fp32"], q
@@ -611,6 +611,6 @@ def test_warm_start_and_ragged_batch_fp32_tc_path():
     for q in range(3):
         o = o12[q]
         for _ in range(4):
-            o = reconstruct(od, b[q], ic[q], 1, psi0=o["psi"])
+            o = reconstruct(od, b[q], ic[q], 1, psi0=o["psi"], X0=o["X"])
         assert psi_rel_err(out["psi"][q], o["psi"]) <= PSI_TOL["fp32"], q
     rec.close()
