@@ -10,9 +10,9 @@ MU0 = 4.0e-7 * np.pi
 
 # name -> config (BASELINE.json configs[0..4])
 CONFIGS = {
-    "cfg1": dict(idx=1, n=33, zmax=1.5, n_probe=40, n_loop=20, n_pf=8, n_eddy=0, n_p=2, n_ff=2,
+    "cfg1": dict(idx=1, lam=0.003, n=33, zmax=1.5, n_probe=40, n_loop=20, n_pf=8, n_eddy=0, n_p=2, n_ff=2,
                  batch=1, n_iter=10, precision="fp64", ic_range=20e3, shapes=("limited",)),
-    "cfg2": dict(idx=2, n=65, zmax=1.5, n_probe=76, n_loop=34, n_pf=12, n_eddy=0, n_p=3, n_ff=3,
+    "cfg2": dict(idx=2, lam=0.003, n=65, zmax=1.5, n_probe=76, n_loop=34, n_pf=12, n_eddy=0, n_p=3, n_ff=3,
                  batch=1, n_iter=15, precision="fp32", ic_range=20e3, shapes=("limited",)),
     "cfg3": dict(idx=3, n=129, zmax=1.6, n_probe=100, n_loop=40, n_pf=16, n_eddy=0, n_p=3, n_ff=3,
                  batch=1, n_iter=20, precision="fp32", ic_range=30e3, shapes=("lsn",)),
@@ -132,7 +132,7 @@ def make_device(name, with_tables=True):
                 cold_rc=0.80, cold_zc=0.0, cold_a=0.40, cold_b=0.72)
     meta = dict(cfg=c, name=name, r=r, z=z, sen_r=sen_r, sen_z=sen_z, alpha=alpha, n_probe=c["n_probe"],
                 src_r=src_r, src_z=src_z, src_w=src_w, n_pf=c["n_pf"])
-    basis = dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=LAMBDA_REG, delz=1, relax=RELAX)
+    basis = dict(n_p=c["n_p"], n_ff=c["n_ff"], lambda_reg=c.get("lam", LAMBDA_REG), delz=1, relax=RELAX)
     if c.get("spline"):
         # BASELINE.json configs[4]: "plus 5-knot tension-spline FF' edge terms" (7 knots
         # 0.70 .. 1.00, tension 10, the five interior cardinal functions)
