@@ -14,8 +14,9 @@ discretisation (PAPER.md:118-120):
            ->  psi = psi_pl + G_GC I_C  ->  oracle.search (axis, X-point, LCFS, psi_N) }
 until the flux stops changing.  Measurements b = G_P I + G_C I_C of the converged state + Gaussian
 noise, sigma = 0.5 % of the RMS of the channel group (probes / loops) over the batch.
-A seed is accepted when the oracle's own reconstruction from the cold start ends with status 0 and
-contracts; otherwise the next seed is tried (rejections are recorded in the file).
+A seed is accepted when the oracle's own reconstruction from the cold start ends with status 0, has the
+labelled boundary type, contracts, and (FP32 configs) is well posed: rounding all inputs to FP32 moves the
+coefficients by at most 3e-6; otherwise the next seed is tried (rejections are recorded in the file).
 """
 import argparse
 import os
@@ -190,17 +191,38 @@ def _design_until_ok(seed):
         nfail += 1
 
 
+def _r32(a):
+    return np.asarray(a, np.float32).astype(np.float64)
+
+
+def _coef_change(Xa, Xb, n_p, dz):
+    """Largest coefficient change relative to the largest coefficient of its kind (delz: relative to dZ)."""
+    npoly = len(Xa) - 1
+    e = max(np.max(np.abs(Xa[:n_p] - Xb[:n_p])) / np.max(np.abs(Xb[:n_p])),
+            np.max(np.abs(Xa[n_p:npoly] - Xb[n_p:npoly])) / np.max(np.abs(Xb[n_p:npoly])))
+    return float(max(e, abs(Xa[-1] - Xb[-1]) / dz))
+
+
 def _accept_job(args):
     k, b, ic, sigma = args
     dev = _W["dev"]
     c = dev["meta"]["cfg"]
-    g = dict(dev["geom"]); g["sigma"] = sigma
-    od = Device(dev["grid"], g, dev["tables"], dev["basis"]) if _W.get("od_sig") is None else _W["od_sig"]
-    _W["od_sig"] = od
+    if _W.get("od_sig") is None:
+        g = dict(dev["geom"]); g["sigma"] = sigma
+        _W["od_sig"] = Device(dev["grid"], g, dev["tables"], dev["basis"])
+        if c["precision"] == "fp32":      # the same device with the tables rounded to FP32 (what the FP32 path sees)
+            _W["od_32"] = Device(dev["grid"], g, {kk: _r32(v) for kk, v in dev["tables"].items()}, dev["basis"])
+    od = _W["od_sig"]
     res = reconstruct(od, b, ic, c["n_iter"], trace=True)
     dp = [h["dpsi"] for h in res["hist"]]
     rate = (dp[-1] / dp[-6]) ** 0.2 if len(dp) >= 7 and dp[-6] > 0 else 1.0
-    return k, res["status"], rate, float(res["chi2"]) if res["status"] == 0 else np.nan, (res["srch"]["limited"] if res["srch"] else -1)
+    sens = 0.0
+    if res["status"] == 0 and c["precision"] == "fp32":
+        # well-posedness for an FP32 path: rounding every input to FP32 (a 6e-8 perturbation) must not move the
+        # coefficients by more than 3e-6 of their kind, else 1e-4 parity of an FP32 pipeline cannot be judged on this slice
+        r2 = reconstruct(_W["od_32"], _r32(b), _r32(ic), c["n_iter"])
+        sens = _coef_change(r2["X"], res["X"], od.n_p, od.op.dz) if r2["status"] == 0 else 1.0
+    return k, res["status"], rate, float(res["chi2"]) if res["status"] == 0 else np.nan, (res["srch"]["limited"] if res["srch"] else -1), sens
 
 
 def generate(cfg, jobs):
@@ -242,13 +264,13 @@ def generate(cfg, jobs):
         while todo:
             res = list(ex.map(_accept_job, [(s, b[s], out[s][1]["ic"], sigma) for s in todo], chunksize=1))
             redo = []
-            for s, (_, st, rate, chi2, lim) in zip(todo, res):
+            for s, (_, st, rate, chi2, lim, sens) in zip(todo, res):
                 want_div = out[s][1]["kind"] != "limited"
-                ok = st == 0 and rate < 0.8 and (lim == 0) == want_div
+                ok = st == 0 and rate < 0.8 and (lim == 0) == want_div and sens <= 3e-6
                 if ok:
                     stats[s] = (rate, chi2, lim)
                 else:
-                    rejected.append((s, out[s][0], f"accept status={st} rate={rate:.2f} limited={lim}"))
+                    rejected.append((s, out[s][0], f"accept status={st} rate={rate:.2f} limited={lim} sens={sens:.1e}"))
                     redo.append(s)
             # replacement seeds for the rejected slots, designed in parallel (a worker keeps trying seed + 10000 k)
             new = list(ex.map(_design_until_ok, [out[s][0] + 10000 for s in redo], chunksize=1))
