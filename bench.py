@@ -406,6 +406,18 @@ def latency_batch1(args, torch, P):
         e0.record(); rec.reconstruct(d_b, d_ic, 1, warm_start=True); e1.record()
         torch.cuda.synchronize()
         tw.append(e0.elapsed_time(e1))
+    # flux-surface post-processing of the paper's timing (33 profile points; Sec. II.E): 33 levels x 128
+    # chords, 10 bisections, three Q integrals, q profile, LCFS geometry -- a separate call (ptefit_flux_surfaces)
+    for _ in range(3):
+        rec.flux_surfaces(1, n_prof=33, n_chord=128, n_bisect=10, f_vac=2.5e6, want_vert=False)
+    torch.cuda.synchronize()
+    tf = []
+    for _ in range(30):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); rec.flux_surfaces(1, n_prof=33, n_chord=128, n_bisect=10, f_vac=2.5e6, want_vert=False); e1.record()
+        torch.cuda.synchronize()
+        tf.append(e0.elapsed_time(e1))
+    us_flux = 1e3 * float(np.median(tf))
     # streaming replay (PAPER.md:158, 175 / Fig. 3): 10 000 consecutive slices, one warm-started Picard
     # iteration each (the previous slice's flux is the start), measurements cycling through the stored
     # cfg3 slices; one event pair per slice, read after the loop
@@ -438,7 +450,8 @@ def latency_batch1(args, torch, P):
     rec.close()
     return dict(workload="cfg3", streaming=stream, us_per_slice=1e3 * float(np.median(ts)), us_min=1e3 * float(min(ts)), n_iter=c["n_iter"],
                 us_per_iteration=1e3 * float(np.median(ts)) / c["n_iter"],
-                us_one_warm_iteration=1e3 * float(np.median(tw)),
+                us_one_warm_iteration=1e3 * float(np.median(tw)), us_flux_surfaces=us_flux,
+                us_warm_iteration_plus_flux_surfaces=1e3 * float(np.median(tw)) + us_flux,
                 launches_per_call=n, paper_context="0.268 ms/slice at 129x129 on the paper's GPU (PAPER.md:175), other hardware")
 
 

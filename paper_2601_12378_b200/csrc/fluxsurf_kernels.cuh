@@ -23,11 +23,19 @@ struct FsSpec {
   double f_vac;
 };
 
+// x^e for a small integer exponent (Eq. 12's mu, nu): multiplications and one reciprocal instead of pow().
+__device__ __forceinline__ double fs_ipow(double x, int e) {
+  double p = 1.0;
+  const int n = e < 0 ? -e : e;
+  for (int k = 0; k < n; ++k) p *= x;
+  return e < 0 ? 1.0 / p : p;
+}
+
 template <typename T>
 struct FsField {
   const T *psi, *xn;
   int nr, nz;
-  double rmin, zmin, dr, dz, rmax, zmax, pa, inv;
+  double rmin, zmin, dr, dz, rmax, zmax, pa, inv, idr, idz;
   __device__ __forceinline__ double F(int n) const {
     const double x = (double)xn[n];
     return x >= 0.0 ? x : fmax(((double)psi[n] - pa) * inv, 1.0);
@@ -38,15 +46,21 @@ struct FsField {
     i0 = max(0, min(i0, nr - 2)); j0 = max(0, min(j0, nz - 2));
     tx = fi - i0; ty = fj - j0; n0 = j0 * nr + i0;
   }
+  // the filtered field is continuous across cell edges, so the cell may be found with reciprocal spacings here
+  // (cell() keeps the divisions: the gradient of the interpolant is not continuous)
   __device__ __forceinline__ double Fat(double R, double Z) const {
-    int n0; double tx, ty;
-    cell(R, Z, n0, tx, ty);
+    const double fi = (R - rmin) * idr, fj = (Z - zmin) * idz;
+    int i0 = (int)floor(fi), j0 = (int)floor(fj);
+    i0 = max(0, min(i0, nr - 2)); j0 = max(0, min(j0, nz - 2));
+    const double tx = fi - i0, ty = fj - j0;
+    const int n0 = j0 * nr + i0;
     return (1.0 - ty) * ((1.0 - tx) * F(n0) + tx * F(n0 + 1)) + ty * ((1.0 - tx) * F(n0 + nr) + tx * F(n0 + nr + 1));
   }
   __device__ __forceinline__ bool inside(double R, double Z) const { return R > rmin && R < rmax && Z > zmin && Z < zmax; }
 };
 
-// grid B, block FS_THREADS, dyn smem (n_chord + 2 n_prof n_chord) doubles.
+// grid (B, G): CTA (s, g) handles the levels p = g, g + G, ... of slice s (every CTA repeats the cheap marching
+// phase; the CTA that owns the last level writes the geometry).  block FS_THREADS, dyn smem (n_chord + 2 n_prof n_chord) doubles.
 // Q[B][n_prof][n_q], q[B][n_prof], geom[B][6], vert[B][n_prof][n_chord][2] (may be nullptr), fstat[B].
 template <typename T>
 __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S, const T *__restrict__ psi_all, T *__restrict__ Qo,
@@ -58,10 +72,12 @@ __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S
   double *vz = vr + (size_t)S.n_prof * S.n_chord;                  // [n_prof][n_chord] vertex Z
   __shared__ int sh_bad;
   const int s = blockIdx.x, tid = threadIdx.x, nth = blockDim.x, lane = tid & 31, warp = tid >> 5;
+  const int G = gridDim.y, g0 = blockIdx.y;
+  const int npl = g0 < S.n_prof ? (S.n_prof - 1 - g0) / G + 1 : 0;          // levels of this CTA: p = g0 + k G, k < npl
   const SearchOut so = D.so[s];
   FsField<T> f;
   f.psi = psi_all + (size_t)s * D.N; f.xn = D.xn + (size_t)s * D.N; f.nr = D.nr; f.nz = D.nz;
-  f.rmin = D.rmin; f.zmin = D.zmin; f.dr = D.dr; f.dz = D.dz;
+  f.rmin = D.rmin; f.zmin = D.zmin; f.dr = D.dr; f.dz = D.dz; f.idr = 1.0 / D.dr; f.idz = 1.0 / D.dz;
   f.rmax = D.rmin + (D.nr - 1) * D.dr; f.zmax = D.zmin + (D.nz - 1) * D.dz;
   f.pa = so.axis_psi; f.inv = 1.0 / (so.psi_b - so.axis_psi);
   const double Ra = so.axis_r, Za = so.axis_z;
@@ -70,22 +86,26 @@ __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S
   if (tid == 0) sh_bad = D.status[s] != 0 ? 1 : 0;
   __syncthreads();
   const bool dead = sh_bad != 0;
-  if (!dead)
-    for (int c = tid; c < S.n_chord; c += nth) {
+  if (!dead)                                           // one warp per chord: 32 marching steps at a time, first hit by ballot
+    for (int c = warp; c < S.n_chord; c += nth >> 5) {
       const double th = two_pi * c / S.n_chord, ct = cos(th), st = sin(th);
-      int k = 1;
-      while (true) {
-        const double R = Ra + k * h * ct, Z = Za + k * h * st;
-        if (!f.inside(R, Z) || f.Fat(R, Z) >= 1.0) break;
-        ++k;
+      int k = 0;
+      for (int base = 1; k == 0; base += 32) {
+        const int kk = base + lane;
+        const double R = Ra + kk * h * ct, Z = Za + kk * h * st;
+        const bool hit = !f.inside(R, Z) || f.Fat(R, Z) >= 1.0;
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        if (m) k = base + __ffs(m) - 1;
       }
-      tb[c] = k * h;
-      if (k == 1 && f.Fat(Ra, Za) >= 1.0) sh_bad = 2;
+      if (lane == 0) {
+        tb[c] = k * h;
+        if (k == 1 && f.Fat(Ra, Za) >= 1.0) sh_bad = 2;
+      }
     }
   __syncthreads();
   if (!dead)
-    for (int e = tid; e < S.n_prof * S.n_chord; e += nth) {
-      const int p = e / S.n_chord, c = e - p * S.n_chord;
+    for (int e0 = tid; e0 < npl * S.n_chord; e0 += nth) {
+      const int pk = e0 / S.n_chord, c = e0 - pk * S.n_chord, p = g0 + pk * G, e = p * S.n_chord + c;
       const double th = two_pi * c / S.n_chord, ct = cos(th), st = sin(th);
       const double x = (p + 1.0) / S.n_prof;
       double lo = 0.0, hi = tb[c];
@@ -107,7 +127,8 @@ __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S
   __syncthreads();
   // closed integrals: one warp per level, lanes over polygon edges
   const double *X = D.X + (size_t)s * D.nt;
-  for (int p = warp; p < S.n_prof; p += nth >> 5) {
+  for (int pk = warp; pk < npl; pk += nth >> 5) {
+    const int p = g0 + pk * G;
     double acc[FS_MAX_Q];
 #pragma unroll
     for (int e = 0; e < FS_MAX_Q; ++e) acc[e] = 0.0;
@@ -129,7 +150,7 @@ __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S
         const double dl = sqrt(dRl * dRl + dZl * dZl);
 #pragma unroll
         for (int e = 0; e < FS_MAX_Q; ++e)
-          if (e < S.n_q) acc[e] += 0.5 * (pow(gv[0], (double)S.mu[e]) * pow(Rv[0], (double)S.nu[e]) + pow(gv[1], (double)S.mu[e]) * pow(Rv[1], (double)S.nu[e])) * dl;
+          if (e < S.n_q) acc[e] += 0.5 * (fs_ipow(gv[0], S.mu[e]) * fs_ipow(Rv[0], S.nu[e]) + fs_ipow(gv[1], S.mu[e]) * fs_ipow(Rv[1], S.nu[e])) * dl;
       }
 #pragma unroll
     for (int e = 0; e < FS_MAX_Q; ++e) acc[e] = warp_sum(acc[e]);
@@ -148,7 +169,7 @@ __global__ void __launch_bounds__(FS_THREADS) k_flux_surfaces(Dev<T> D, FsSpec S
     }
   }
   // LCFS geometry (last level): R_min, R_max, Z_min, Z_max, a, kappa
-  if (warp == 0) {
+  if (warp == 0 && (S.n_prof - 1) % G == g0) {
     double rmin = INFINITY, rmax = -INFINITY, zmin = INFINITY, zmax = -INFINITY;
     if (!dead)
       for (int c = lane; c < S.n_chord; c += 32) {

@@ -350,6 +350,10 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   }
   // workspaces
   TRY(dev_alloc(h, &D.xn, (size_t)B * N));
+  {   // -1 = outside the plasma: the lean search kernels rewrite the lim_mask words only
+    std::vector<T> m1(N, T(-1));
+    for (int q = 0; q < B; ++q) CK(cudaMemcpy(D.xn + (size_t)q * N, m1.data(), N * sizeof(T), cudaMemcpyHostToDevice));
+  }
   TRY(dev_alloc(h, &D.psi_coil, (size_t)B * N));
   TRY(dev_alloc(h, &D.dred, (size_t)B * D.M));
   TRY(dev_alloc(h, &D.resp, (size_t)B * D.M * D.nt));
@@ -501,7 +505,11 @@ ptefit_status flux_surfaces(ptefit_handle *h, Dev<T> &D, int B, const ptefit_pro
   if (S.ff0 < 0) S.ff0 = 0;
   const size_t sm = ((size_t)S.n_chord + 2 * (size_t)S.n_prof * S.n_chord) * sizeof(double);
   CK(cudaFuncSetAttribute(k_flux_surfaces<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-  k_flux_surfaces<T><<<B, FS_THREADS, sm, st>>>(D, S, psi, Q, q, geom, vert, fstat);
+  // few slices: spread the levels of a slice over several CTAs
+  int G = B >= 2 * h->nsm ? 1 : (2 * h->nsm + B - 1) / B;
+  if (G > S.n_prof) G = S.n_prof;
+  if (G > 16) G = 16;
+  k_flux_surfaces<T><<<dim3(B, G), FS_THREADS, sm, st>>>(D, S, psi, Q, q, geom, vert, fstat);
   CK(cudaGetLastError());
   return PTEFIT_OK;
 }

@@ -495,4 +495,43 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   if (warp == 0) tc::tmem_dealloc<512>(tmem_base);
 }
 
+// Stand-alone lean search for warm starts on the FP32 tensor-core path: flux map into shared memory, then
+// search_lean (normalised flux on the lim_mask words; the rest of xn keeps the -1 written at create).
+// grid B, block TCS_THREADS, dyn smem tcs_search_smem_bytes.
+__host__ __device__ inline size_t tcs_search_smem_bytes(int nr, int nz) {
+  const size_t N = (size_t)nr * nz, nwords = (N + 31) / 32;
+  return (N + 4) * sizeof(float) + 4 * nwords * sizeof(unsigned) + 4 * nwords * sizeof(unsigned short) + 64;
+}
+__global__ void __launch_bounds__(TCS_THREADS, 1) k_search_tc(Dev<float> D, TcSolveDev S, const float *__restrict__ psi_all, float *__restrict__ xn_all) {
+  extern __shared__ __align__(16) unsigned char smem_dyn[];
+  __shared__ LeanShared lean;
+  if (!psi_all) psi_all = reinterpret_cast<const float *>(D.ca->psi);
+  const int s = blockIdx.x, tid = threadIdx.x, nth = blockDim.x, N = D.N, nwords = (N + 31) >> 5;
+  float *G = reinterpret_cast<float *>(smem_dyn);
+  unsigned *mbits = reinterpret_cast<unsigned *>(G + ((N + 3) & ~3));
+  unsigned short *wls = reinterpret_cast<unsigned short *>(mbits + 4 * nwords);
+  for (int w = tid; w < 4 * nwords; w += nth) {
+    mbits[w] = (w < nwords) ? D.lim_bits[w] : (w < 2 * nwords) ? D.xpt_bits[w - nwords] : (w < 3 * nwords) ? D.dil_bits[w - 2 * nwords] : D.dil2_bits[w - 3 * nwords];
+    wls[w] = S.wl[w];
+  }
+  WordLists WL;
+  WL.lim = wls; WL.xpt = wls + nwords; WL.dil = wls + 2 * nwords; WL.zero = wls + 3 * nwords;
+  WL.n_lim = S.n_lim; WL.n_xpt = S.n_xpt; WL.n_dil = S.n_dil; WL.n_zero = S.n_zero;
+  __syncthreads();
+  const float *psi = psi_all + (size_t)s * N;
+  const float sgT = float(D.ip_sign);
+  float am_v = -INFINITY, chk = 0.f;
+  int am_n = 0x7fffffff;
+  for (int n = tid; n < N; n += nth) {
+    const float v = psi[n];
+    G[n] = v;
+    chk = fmaf(v, 0.f, chk);
+    const float key = sgT * v;
+    if (((mbits[n >> 5] >> (n & 31)) & 1u) && key > am_v) { am_v = key; am_n = n; }      // n increases per thread: ties keep the smallest
+  }
+  __syncthreads();
+  search_lean(D, lean, s, G, xn_all + (size_t)s * N, mbits, mbits + nwords, mbits + 3 * nwords, WL, am_v, am_n, !(chk == 0.f), nullptr, nullptr,
+              nullptr, nullptr);
+}
+
 }  // namespace ptefit
