@@ -333,7 +333,7 @@ def run_ours(args):
                us_per_slice_iteration=1e3 * total_ms / args.steps / B / max(n_iter, 1), higher_is_better=True,
                scaling="weak", vs_baseline=None, dtype="f32" if prec == "fp32" else "f64", data="synthetic",
                config=dict(workload=args.config, grid=f"{rec.nr}x{rec.nz}", batch_per_gpu=B, n_iter=n_iter, n_meas=rec.M,
-                           n_coil=rec.nc, n_terms=rec.nt, unique_slices=n_unique, gemm=args.gemm,
+                           n_coil=rec.nc, n_terms=rec.nt, unique_slices=n_unique, gemm=args.gemm if prec == "fp32" else "fp64-dmma",
                            l2="flushed between timed steps (256 MB memset) and working set > L2",
                            parallelism=f"slices sharded over {world} GPU(s), no collective"),
                clocks=clocks, e2e=e2e, gpu_launches=launches, slices_status_ok=n_ok, roofline=roof,
