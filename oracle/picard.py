@@ -82,10 +82,12 @@ def picard_iteration(dev, psin, mask, d, psi_coil, X_prev=None, psi_prev=None, b
     return out
 
 
-def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False, X0=None):
+def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False, X0=None, psi_noise=None):
     """ptefit_reconstruct for one slice.  psi0 = None -> cold start (O2), else warm start; X0 = the
     coefficients of the previous call (a warm start keeps them: they seed the vertical-shift column of the
-    first iteration, which is what keeps the one-iteration-per-slice mode of PAPER.md:158 from drifting)."""
+    first iteration, which is what keeps the one-iteration-per-slice mode of PAPER.md:158 from drifting).
+    psi_noise = (rel, seed): test hook of the case generator -- Gaussian noise of rel * max|psi| is added to the
+    flux after every iteration, to see whether a slice's decisions survive FP32-level perturbations."""
     d = np.asarray(b, np.float64) - dev.gc @ np.asarray(ic, np.float64)           # Eq. 2 / Eq. 6 rhs
     psi_coil = (dev.ggc @ np.asarray(ic, np.float64)).reshape(dev.nz, dev.nr)
     res = dict(status=0, X=np.zeros(dev.nb) if (X0 is None or psi0 is None) else np.array(X0, np.float64), chi2=np.nan, psi=None,
@@ -111,6 +113,11 @@ def reconstruct(dev, b, ic, n_iter, psi0=None, trace=False, X0=None):
         if "ic_fit" in o:
             res["ic_fit"] = o["ic_fit"]
         res["X"], res["chi2"], res["status"] = o["X"], o["chi2"], o["status"]
+        if "psi" in o and psi_noise is not None and o["status"] == 0:
+            rng = np.random.default_rng(psi_noise[1] + 1000 * it)
+            o["psi"] = o["psi"] + psi_noise[0] * np.max(np.abs(o["psi"])) * rng.standard_normal(o["psi"].shape)
+            o["srch"] = _search.search(o["psi"], dev.r, dev.z, dev.lim_mask, dev.xpt_mask, dev.lim_r, dev.lim_z, dev.s)
+            o["status"] = o["srch"]["status"]
         if "psi" in o:
             if trace:
                 res["hist"].append(dict(X=o["X"], chi2=o["chi2"], dpsi=float(np.max(np.abs(o["psi"] - res["psi"]))),

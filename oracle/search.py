@@ -66,7 +66,7 @@ def search(psi, r, z, lim_mask, xpt_mask, lim_r, lim_z, s=1):
     dr, dz = r[1] - r[0], z[1] - z[0]
     out = dict(status=0, axis=(-1, -1, np.nan, np.nan, np.nan), xpt=(-1, -1, np.nan, np.nan, np.nan),
                psi_b=np.nan, limited=1, mask=np.zeros((nz, nr), bool), psin=np.zeros((nz, nr)),
-               axis_margin=np.nan, xpt_margin=np.nan, n_cand=0)
+               axis_margin=np.nan, xpt_margin=np.nan, n_cand=0, bnd_margin=np.inf, valid_margin=np.inf)
     if not np.all(np.isfinite(psi)):
         out["status"] = 2
         return out
@@ -111,6 +111,23 @@ def search(psi, r, z, lim_mask, xpt_mask, lim_r, lim_z, s=1):
     if not np.isfinite(spb):
         out["status"] = 1
         return out
+    # decision margins (diagnostics only; the case generator rejects seeds whose decisions are fragile):
+    # bnd_margin = gap between the best X-point and the best valid limiter vertex; valid_margin = how far the
+    # half-plane test of a vertex that matters is from flipping (normalised dot product): vertices above the
+    # boundary flux are all invalid -- the least firmly invalid one counts -- and so does the winning vertex.
+    scale0 = abs(psia - s * spb)
+    out["bnd_margin"] = abs(best_x - best_lim) / scale0 if (np.isfinite(best_x) and np.isfinite(best_lim) and scale0 > 0) else np.inf
+    vm = np.inf
+    if len(ci):
+        dots = np.stack([((lim_r - cR[c]) * (Ra - cR[c]) + (lim_z - cZ[c]) * (Za - cZ[c]))
+                         / (np.hypot(lim_r - cR[c], lim_z - cZ[c]) * np.hypot(Ra - cR[c], Za - cZ[c]) + 1e-300) for c in range(len(ci))])
+        above = (~valid) & (s * pv > spb)
+        if above.any():
+            vm = min(vm, float(np.min(-np.min(dots[:, above], axis=0))))      # most negative dot of each such vertex
+        if out["limited"] == 1 and valid.any():
+            kw = int(np.argmax(np.where(valid, s * pv, -np.inf)))
+            vm = min(vm, float(np.min(dots[:, kw])))
+    out["valid_margin"] = vm
     psib = s * spb
     out["psi_b"] = psib
     # 5. plasma region

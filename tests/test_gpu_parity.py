@@ -614,3 +614,29 @@ def test_warm_start_and_ragged_batch_fp32_tc_path():
             o = reconstruct(od, b[q], ic[q], 1, psi0=o["psi"], X0=o["X"])
         assert psi_rel_err(out["psi"][q], o["psi"]) <= PSI_TOL["fp32"], q
     rec.close()
+
+
+def test_cfg4_every_slice_of_the_batch_against_oracle():
+    """BASELINE config 4 exactly as bench.py times it (512 distinct designed slices, max_batch 512, 20
+    iterations): EVERY slice against the oracle (about 80 s of oracle time), with the figures printed."""
+    torch = _torch()
+    dev, sl = cached_case("cfg4", 512)
+    dv, b, ic = round_inputs(dev, sl, "fp32")
+    od = oracle_device(dv)
+    rec = _rec(dev, "fp32", 512)
+    rec.reconstruct(torch.tensor(b, dtype=rec.dtype, device="cuda"), torch.tensor(ic, dtype=rec.dtype, device="cuda"), 20)
+    torch.cuda.synchronize()
+    out = _gpu_out(rec, 512)
+    loose = 0
+    worst = dict(psi=0.0, coef=0.0, coef_each=0.0, coef_each_all=0.0)
+    for q in range(512):
+        ores = reconstruct(od, b[q], ic[q], 20)
+        assert ores["status"] == 0, q
+        r = check_slice(out, q, ores, dev, "fp32", strict_index=False)
+        loose += (not r["index_ok"])
+        for k in worst:
+            worst[k] = max(worst[k], r[k])
+    print(f"cfg4 all 512 slices: near-tie index clause used by {loose}; worst psi {worst['psi']:.2e}, coefficients per kind {worst['coef']:.2e}, "
+          f"per coefficient (>= 10 % of its kind) {worst['coef_each']:.2e}, per coefficient (all) {worst['coef_each_all']:.2e}")
+    assert loose <= 2
+    rec.close()
