@@ -211,6 +211,28 @@ ptefit_status ptefit_greens_table(int n_fld, const double *d_fld_r, const double
                                   int n_src, const double *d_src_r, const double *d_src_z,
                                   const double *d_src_w, double *d_out, int transpose, void *cuda_stream);
 
+/* Allocation-free Delta* solve (Eq. 1; Sec. II.C), for callers that must not
+ * allocate (CUDA graph capture, serving loops): the same operation as ptefit_debug_gs_solve,
+ *   psi[batch][nz][nr] = solve(-mu0 R I / dA with edge data psi_bdry[batch][n_bnd]),
+ * on the FP64 DMMA route (transposed right-hand side, DST in Z as a tensor-core product, FP64 Thomas in R,
+ * inverse DST, transpose back) with ALL of that route's workspace -- three transposed maps and the Thomas
+ * forward-sweep values, batch * (nr-2) * (3 * ld + nz-2) doubles, ld = nz-2 rounded up to even -- in one
+ * file-scope __device__ array of PTEFIT_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds
+ * until exit.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine (the first
+ * call on a device resolves the array's device address with cudaGetSymbolAddress, which allocates nothing).
+ * h: an FP64 handle whose contractions are not FFMA (it supplies the DST matrix and the tridiagonal factors,
+ * which were copied at ptefit_create); the device of h must be current.  d_I[batch][nz*nr], d_psi_bdry and
+ * d_psi are caller-owned DEVICE memory, FP64.  Asynchronous on cuda_stream.
+ * Errors: PTEFIT_ERR_UNSUPPORTED for an FP32 / FFMA handle; PTEFIT_ERR_INVALID_ARG with a message that names
+ * the need and the limit when the workspace of `batch` slices exceeds PTEFIT_NOALLOC_SCRATCH_BYTES (the limit
+ * is 65 slices at 65x65, 16 at 129x129, 4 at 257x257) -- nothing is launched then.
+ * The array is shared by every call, every handle and every stream of the process on that GPU and keeps the
+ * last call's contents; the call clears the part it uses first.  Calls that overlap on the GPU (different
+ * streams, or the same call replayed concurrently from a graph) race on it: serialise them. */
+#define PTEFIT_NOALLOC_SCRATCH_BYTES (8u << 20)
+ptefit_status ptefit_gs_solve_noalloc(ptefit_handle *h, int batch, const double *d_I, const double *d_psi_bdry,
+                                      double *d_psi, void *cuda_stream);
+
 void ptefit_destroy(ptefit_handle *h);
 const char *ptefit_last_error(const ptefit_handle *h);
 const char *ptefit_global_error(void);

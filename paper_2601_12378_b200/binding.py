@@ -12,12 +12,14 @@ EXPORTED_SYMBOLS = [
     "ptefit_create", "ptefit_reconstruct", "ptefit_reconstruct_host", "ptefit_destroy", "ptefit_last_error",
     "ptefit_global_error", "ptefit_debug_gs_solve", "ptefit_debug_search", "ptefit_debug_fit",
     "ptefit_last_launch_count", "ptefit_set_profiling", "ptefit_get_stage_ms", "ptefit_greens_table", "ptefit_get_coil_currents", "ptefit_flux_surfaces",
+    "ptefit_gs_solve_noalloc",
 ]
 
 PTEFIT_FP32, PTEFIT_FP64 = 0, 1
 GEMM_3XTF32, GEMM_FFMA = 0, 2
 OPT_NO_GRAPH, OPT_NO_FUSED_BASIS, OPT_SOLVE_FFMA = 1, 2, 4
 FAMILY_POLY, FAMILY_SPLINE = 0, 1
+NOALLOC_SCRATCH_BYTES = 8 << 20   # PTEFIT_NOALLOC_SCRATCH_BYTES of include/ptefit.h
 
 
 class PtefitError(RuntimeError):
@@ -85,6 +87,8 @@ def load_library():
         lib.ptefit_global_error.restype = C.c_char_p
         lib.ptefit_debug_gs_solve.restype = C.c_int
         lib.ptefit_debug_gs_solve.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
+        lib.ptefit_gs_solve_noalloc.restype = C.c_int
+        lib.ptefit_gs_solve_noalloc.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 4
         lib.ptefit_debug_search.restype = C.c_int
         lib.ptefit_debug_search.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 10
         lib.ptefit_debug_fit.restype = C.c_int
@@ -254,6 +258,12 @@ class Reconstructor:
     def debug_gs_solve(self, d_I, d_pbd, d_psi_out):
         s = self.torch.cuda.current_stream()
         self._call(self.lib.ptefit_debug_gs_solve, d_I.shape[0], _dp(d_I), _dp(d_pbd), _dp(d_psi_out), C.c_void_p(s.cuda_stream))
+
+    def gs_solve_noalloc(self, d_I, d_pbd, d_psi_out):
+        """ptefit_gs_solve_noalloc: the Delta* solve with its workspace in the library's static device array
+        (FP64 handles; at most NOALLOC_SCRATCH_BYTES of workspace per call; no allocation inside the call)."""
+        s = self.torch.cuda.current_stream()
+        self._call(self.lib.ptefit_gs_solve_noalloc, d_I.shape[0], _dp(d_I), _dp(d_pbd), _dp(d_psi_out), C.c_void_p(s.cuda_stream))
 
     def debug_search(self, d_psi, d_xn):
         s = self.torch.cuda.current_stream()

@@ -544,3 +544,98 @@ extern "C" const char *ptefit_global_error(void) { return g_error.c_str(); }
 extern "C" int ptefit_last_launch_count(const ptefit_handle *h) { return h ? h->launches : 0; }
 
 #include "launch.inc"
+
+// ---------------------------------------------------------------------------------------------------------
+// ptefit_gs_solve_noalloc (include/ptefit.h): the GEMM-based FP64 Delta* solve (launch_solve_dm's sequence:
+// PAPER.md:33 Eq. 1) with its whole workspace in one file-scope device array instead of the
+// handle's cudaMalloc'ed buffers.  Every GPU that loads the library holds the array until exit; all calls
+// share it and it keeps the last call's contents.
+// ---------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[PTEFIT_NOALLOC_SCRATCH_BYTES];
+
+namespace ptefit {
+// k_tridiag_ld with both of its work arrays passed in: Thomas sweeps along R in FP64, one thread per
+// (slice, mode), in place on fh[(s, i)][m] (row length ld); forward-sweep values in y[(s, i)][m] (row length
+// nzi).  grid (ceil(nzi/128), B), block 128.
+__global__ void k_tridiag_ld_scratch(Dev<double> D, int ld, double *__restrict__ fh_all, double *__restrict__ y_all) {
+  const int s = blockIdx.y, mm = blockIdx.x * blockDim.x + threadIdx.x;
+  if (mm >= D.nzi) return;
+  const int nri = D.nri, nzi = D.nzi;
+  double *fh = fh_all + (size_t)s * nri * ld;
+  double *y = y_all + (size_t)s * nri * nzi;
+  double prev = 0.0;
+  for (int i = 0; i < nri; ++i) {
+    const double v = fh[(size_t)i * ld + mm] - D.tri_w[(size_t)i * nzi + mm] * prev;
+    y[(size_t)i * nzi + mm] = v;
+    prev = v;
+  }
+  double x = 0.0;
+  for (int i = nri - 1; i >= 0; --i) {
+    x = (y[(size_t)i * nzi + mm] - D.tri_ce[i] * x) * D.tri_invb[(size_t)i * nzi + mm];
+    fh[(size_t)i * ld + mm] = x;
+  }
+}
+}  // namespace ptefit
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mu;
+void *g_noalloc_ptr[NOALLOC_MAX_DEVICES];      // device address of g_noalloc_scratch on device d (0 = not resolved yet)
+
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: resolve it once per
+// device, with that device current.
+ptefit_status noalloc_scratch(ptefit_handle *h, double **out) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(h, PTEFIT_ERR_UNSUPPORTED, "ptefit_gs_solve_noalloc: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void *p = nullptr;
+    CK(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return fail(h, PTEFIT_ERR_CUDA, "ptefit_gs_solve_noalloc: cudaGetSymbolAddress returned a null address");
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = reinterpret_cast<double *>(g_noalloc_ptr[dev]);
+  return PTEFIT_OK;
+}
+}  // namespace
+
+extern "C" ptefit_status ptefit_gs_solve_noalloc(ptefit_handle *h, int batch, const double *d_I, const double *d_pbd, double *d_psi,
+                                                 void *cuda_stream) {
+  if (!h) return fail(h, PTEFIT_ERR_INVALID_ARG, "null handle");
+  if (batch < 1) return fail(h, PTEFIT_ERR_INVALID_ARG, "batch must be >= 1");
+  if (!d_I || !d_pbd || !d_psi) return fail(h, PTEFIT_ERR_INVALID_ARG, "null buffer");
+  if (h->prec != PTEFIT_FP64 || !h->dm)
+    return fail(h, PTEFIT_ERR_UNSUPPORTED, "ptefit_gs_solve_noalloc needs an FP64 handle whose contractions are not FFMA");
+  const Dev<double> &D = h->d64;
+  DmDev T = h->Dm;                                   // copy: the three transposed maps move into the static array
+  const size_t n_t = (size_t)batch * D.nri * T.ldS;  // doubles per transposed map (even: 16-byte rows for cp.async)
+  const size_t n_y = (size_t)batch * D.nri * D.nzi;
+  const size_t need = (3 * n_t + n_y) * sizeof(double);
+  if (need > (size_t)PTEFIT_NOALLOC_SCRATCH_BYTES) {
+    char msg[256];
+    snprintf(msg, sizeof msg, "ptefit_gs_solve_noalloc: batch %d on a %d x %d grid needs %zu bytes of scratch, the static array holds %u "
+             "(at most %zu slices of this grid per call)", batch, D.nr, D.nz, need, (unsigned)PTEFIT_NOALLOC_SCRATCH_BYTES,
+             (size_t)PTEFIT_NOALLOC_SCRATCH_BYTES / (((size_t)3 * T.ldS + D.nzi) * D.nri * sizeof(double)));
+    return fail(h, PTEFIT_ERR_INVALID_ARG, msg);
+  }
+  double *s = nullptr;
+  TRY(noalloc_scratch(h, &s));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // the array keeps the previous call's contents: the padding column of the transposed maps (never written by
+  // the kernels below) must read as zero, so the part this call uses is cleared
+  CK(cudaMemsetAsync(s, 0, need, st));
+  T.ft = s; T.fh = s + n_t; T.gt = s + 2 * n_t;
+  double *y = s + 3 * n_t;
+  const dim3 gt((D.nri + 31) / 32, (D.nzi + 31) / 32, batch), bt(32, 8);
+  k_rhs_t<<<gt, bt, 0, st>>>(D, T, d_I, d_pbd);
+  gemm_dmma(T.ft, T.ldS, T.S, T.ldS, T.fh, T.ldS, batch * D.nri, D.nzi, D.nzi, 1, 0, 1.0, st);
+  k_tridiag_ld_scratch<<<dim3((D.nzi + 127) / 128, batch), 128, 0, st>>>(D, T.ldS, T.fh, y);
+  gemm_dmma(T.fh, T.ldS, T.S, T.ldS, T.gt, T.ldS, batch * D.nri, D.nzi, D.nzi, 1, 0, 2.0 / (D.nz - 1), st);
+  k_total_t<<<gt, bt, 0, st>>>(D, T, d_psi, 0, 0);
+  k_edge_total<double><<<dim3((D.nbnd + 255) / 256, batch), 256, 0, st>>>(D, d_psi, d_pbd, 0, 0);
+  CK(cudaGetLastError());
+  return PTEFIT_OK;
+}
