@@ -129,14 +129,21 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
   }
   LS_T(0);
   // 2. X-point candidates: FP32 scan of the xpt_mask words -> compact list (the scan does not need the axis)
-#pragma unroll 2
-  for (int k = warp; k < WL.n_xpt; k += nwarp) {
-    const int w = WL.xpt[k];
-    const int n = (w << 5) + lane;
-    const bool bit = (xbits[w] >> lane) & 1u;
-    if (xpt_prefilter(psi + (bit ? n : nr + 1), nr) && bit) {         // masked-off lanes read a harmless interior node
-      const int q = atomicAdd(&S.nlist, 1);
-      if (q < LEAN_LIST) S.list[q] = n;
+  {                                              // word index and mask word of the next iteration are fetched one iteration ahead
+    int k = warp;
+    int w = k < WL.n_xpt ? WL.xpt[k] : 0;
+    unsigned xb = xbits[w];
+    while (k < WL.n_xpt) {
+      const int kn = k + nwarp;
+      const int wn = kn < WL.n_xpt ? WL.xpt[kn] : 0;
+      const unsigned xbn = xbits[wn];
+      const int n = (w << 5) + lane;
+      const bool bit = (xb >> lane) & 1u;
+      if (xpt_prefilter(psi + (bit ? n : nr + 1), nr) && bit) {         // masked-off lanes read a harmless interior node
+        const int q = atomicAdd(&S.nlist, 1);
+        if (q < LEAN_LIST) S.list[q] = n;
+      }
+      k = kn; w = wn; xb = xbn;
     }
   }
   __syncthreads();
@@ -250,20 +257,45 @@ __device__ __forceinline__ void search_lean(const Dev<float> &D, LeanShared &S, 
 #pragma unroll
     for (int k = 0; k < 5; ++k) { pp[k] = pc ? pc[k] : 0.f; pq[k] = pc ? pc[MD + 1 + k] : 0.f; }
     const bool spl = D.nspl && Xs;
-#pragma unroll 2
-    for (int k = warp; k < WL.n_lim; k += nwarp) {
-      const int w = WL.lim[k];
-      const int n = (w << 5) + lane;
-      const bool bit = (lbits[w] >> lane) & 1u;
+    // half-plane tests of candidates 0 and 1 from registers; an absent candidate reads as "always in front,
+    // never near the margin" (value 1, margin 0).  More than two candidates (rare) take the loop below.
+    const float a0R = ncand > 0 ? S.hR[0] : 0.f, a0Z = ncand > 0 ? S.hZ[0] : 0.f, a00 = ncand > 0 ? S.h0[0] : 1.f, a0m = ncand > 0 ? S.hm[0] : 0.f;
+    const float a1R = ncand > 1 ? S.hR[1] : 0.f, a1Z = ncand > 1 ? S.hZ[1] : 0.f, a10 = ncand > 1 ? S.h0[1] : 1.f, a1m = ncand > 1 ? S.hm[1] : 0.f;
+    int k = warp;
+    int wc = k < WL.n_lim ? WL.lim[k] : 0;
+    unsigned lbc = lbits[wc];
+    float vc = psi[((lbc >> lane) & 1u) ? (wc << 5) + lane : 0];
+    while (k < WL.n_lim) {                            // word index, mask word and flux of the next iteration are fetched one iteration ahead
+      const int w = wc, n = (w << 5) + lane;
+      const bool bit = (lbc >> lane) & 1u;
+      const float v = vc;
+      k += nwarp;
+      wc = k < WL.n_lim ? WL.lim[k] : 0;
+      lbc = lbits[wc];
+      vc = psi[((lbc >> lane) & 1u) ? (wc << 5) + lane : 0];     // read before this iteration's store to psi: different words
+      bool in = bit && (sgf * v > thr);
+      if (!__any_sync(0xffffffffu, in)) {             // no plasma node in this word (warp-uniform): nothing to evaluate
+        if (n < N) { xn[n] = -1.f; psi[n] = pc ? 0.f : -1.f; }
+        continue;
+      }
       const int j = __float2int_rd(((float)n + 0.5f) * inv_nr);     // exact: (n + 0.5)/nr is >= 0.5/nr away from an integer
       const int i = n - j * nr;
-      const float v = psi[bit ? n : 0];
-      bool in = bit && (sgf * v > thr);
-      if (ncand) {                                    // uniform branch
-        for (int c = 0; c < ncand; ++c) {
-          const float val = fmaf(S.hR[c], (float)i, fmaf(S.hZ[c], (float)j, S.h0[c]));
+      const float fi = (float)i, fj = (float)j;
+      {
+        const float v0 = fmaf(a0R, fi, fmaf(a0Z, fj, a00)), v1 = fmaf(a1R, fi, fmaf(a1Z, fj, a10));
+        bool ok0 = v0 > 0.f, ok1 = v1 > 0.f;
+        if (in && (!(fabsf(v0) > a0m) || !(fabsf(v1) > a1m))) {     // inside the FP32 error margin: the FP64 expression decides (rare)
+          const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
+          if (!(fabsf(v0) > a0m)) ok0 = ((R - S.cR[0]) * (Ra - S.cR[0]) + (Z - S.cZ[0]) * (Za - S.cZ[0])) > 0.0;
+          if (!(fabsf(v1) > a1m)) ok1 = ((R - S.cR[1]) * (Ra - S.cR[1]) + (Z - S.cZ[1]) * (Za - S.cZ[1])) > 0.0;
+        }
+        in = in && ok0 && ok1;
+      }
+      if (ncand > 2) {                                // uniform branch
+        for (int c = 2; c < ncand; ++c) {
+          const float val = fmaf(S.hR[c], fi, fmaf(S.hZ[c], fj, S.h0[c]));
           bool ok = val > 0.f;
-          if (in && !(fabsf(val) > S.hm[c])) {        // inside the FP32 error margin: the FP64 expression decides (rare)
+          if (in && !(fabsf(val) > S.hm[c])) {
             const double R = D.rmin + i * D.dr, Z = D.zmin + j * D.dz;
             ok = ((R - S.cR[c]) * (Ra - S.cR[c]) + (Z - S.cZ[c]) * (Za - S.cZ[c])) > 0.0;
           }

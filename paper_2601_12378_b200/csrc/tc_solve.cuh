@@ -40,8 +40,9 @@ constexpr int TCS_TAB_BYTES = 65536;        // sine table hi + lo: 2 x [128][64]
 constexpr int TCS_OP_BYTES = 131072;        // operand tiles: 4 x [128][64] floats (hi / lo x odd / even)
 
 struct TcSolveDev {
-  const double *tcib;         // [128][128] inverse pivots of the Thomas factorisation, [row i][TMEM lane]; rows >= nri are 1
+  const double *tcib;         // [128][128] inverse pivots of the twisted Thomas factorisation, [row i][TMEM lane]; rows >= nri are 1
   const double *tcw, *tce;    // [nri] sub- and super-diagonal of the tridiagonal systems (cw_i, ce_i)
+  int mid;                    // meeting row of the twisted factorisation (top rows < mid, bottom rows > mid)
   const unsigned short *wl;   // [4][nwords] indices of the non-zero words of the lim / xpt / dilated / zero-only masks (WordLists)
   int n_lim, n_xpt, n_dil, n_zero;
 };
@@ -132,9 +133,10 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
   __shared__ T c_rhs[PTEFIT_MAX_NR], c_rdA[PTEFIT_MAX_NR], c_fdA[PTEFIT_MAX_NR];
   __shared__ T pcoef[2 * (PTEFIT_MAX_DEG + 1)];
   __shared__ T c_edge[2];
+  __shared__ double xch[256];                              // Thomas: what the two halves of a mode exchange in the meeting row
   __shared__ LeanShared lean;
   const int tid = threadIdx.x, nth = blockDim.x, warp = tid >> 5, lane = tid & 31;
-  const bool elected = (tid == 4 * 32);                    // lane 0 of warp 4: TMA + MMA issue (warps 0-3 run the Thomas sweeps)
+  const bool elected = (tid == 8 * 32);                    // lane 0 of warp 8: TMA + MMA issue (warps 0-7 run the Thomas sweeps)
 
   if (elected) {
     tc::tma_prefetch_desc(&mapFhi); tc::tma_prefetch_desc(&mapFlo); tc::tma_prefetch_desc(&mapIhi); tc::tma_prefetch_desc(&mapIlo);
@@ -264,66 +266,116 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
       tc::tc_commit(&bar_mma);
     }
     ph_tab ^= 1u;
-    // ---- C. Thomas sweeps along R in FP64, one thread per mode (TMEM lane), warps 0-3.  Normalised form
-    // (unit upper diagonal): z_i = ib_i f_i - (ib_i cw_i) z_{i-1};  x_i = z_i - (ce_i ib_i) x_{i+1}, with
-    // ib = inverse pivots: one table serves both sweeps.  It is staged in the (now free) operand region by
-    // eight bulk copies of 16 rows; z and then x (hi / lo) are parked in TMEM columns 256-511.
-    if (warp < 4) {
+    // ---- C. Thomas sweeps along R in FP64 on the twisted factorisation: two threads per mode (TMEM lane L),
+    // warps 0-3 eliminate downwards from row 0 to row mid-1, warps 4-7 upwards from row nri-1 to row mid+1
+    // (both halves of a lane quarter may touch its TMEM lanes: warp % 4 selects the quarter); they meet in
+    // row mid and substitute back outwards.  Normalised form (unit off-diagonal), ib = inverse pivots of the
+    // respective sweep (row mid: of the meeting row):
+    //   top     z_i = ib_i f_i - (ib_i cw_i) z_{i-1},   x_i = z_i - (ce_i ib_i) x_{i+1}
+    //   bottom  y_i = ib_i f_i - (ib_i ce_i) y_{i+1},   x_i = y_i - (cw_i ib_i) x_{i-1}
+    //   mid     x_m = ib_m (f_m - cw_m z_{m-1} - ce_m y_{m+1}).
+    // The pivot table is staged in the (now free) operand region by eight bulk copies of 16 rows; z / y and
+    // then x are parked in TMEM columns 256-511.  mid + 1 is a multiple of 16 (or mid = nri - 1: no bottom half).
+    if (warp < 8) {
       tc::mbar_wait(&bar_mma, ph_mma);
       tc::tc_fence_after();
       TCS_T(7);
-      const int L = tid;                                   // TMEM lane = mode slot
-      const uint32_t tl = tmem_base + ((uint32_t)(warp * 32) << 16);
+      const int L = tid & 127, half = tid >> 7, mid = S.mid;
+      const bool two = mid + 1 < nri;
+      const uint32_t tl = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
       const uint32_t src = tl + (L < 64 ? 0u : 128u), ya = tl + 256u;
-      double z = 0.0;
-      for (int c = 0; c < 8; ++c) {
-        const int i0 = 16 * c;
-        uint32_t f[16], zlo[16], zhi[16];
-        tmem_ld16u(src + i0, f);
-        TCS_T(10);
-        tc::mbar_wait(&bar_ib[c], ph_ib);
-        TCS_T(11);
+      const int cm = mid >> 4, c_lo = (mid + 1) >> 4, c_hi = (nri - 1) >> 4;
+      if (half == 0) {
+        double z = 0.0, tmid = 0.0;
+        for (int c = 0; c <= cm; ++c) {
+          const int i0 = 16 * c;
+          uint32_t f[16], zlo[16], zhi[16];
+          tmem_ld16u(src + i0, f);
+          tc::mbar_wait(&bar_ib[c], ph_ib);
 #pragma unroll
-        for (int u = 0; u < 16; ++u) {
-          const int i = i0 + u;
-          const double ib = ibs[i * 128 + L];
-          const double v = fma(-(ib * cw_s[i]), z, ib * (double)__uint_as_float(f[u]));
-          z = (i < nri) ? v : z;
-          zlo[u] = (uint32_t)__double2loint(v);
-          zhi[u] = (uint32_t)__double2hiint(v);
+          for (int u = 0; u < 16; ++u) {
+            const int i = i0 + u;
+            const double ib = ibs[i * 128 + L], fi = (double)__uint_as_float(f[u]);
+            const double v = fma(-(ib * cw_s[i]), z, ib * fi);
+            if (i == mid) tmid = fma(-cw_s[i], z, fi);
+            z = (i < mid) ? v : z;
+            zlo[u] = (uint32_t)__double2loint(v);
+            zhi[u] = (uint32_t)__double2hiint(v);
+          }
+          tmem_st16(ya + i0, zlo);
+          tmem_st16(ya + 128 + i0, zhi);
         }
-        tmem_st16(ya + i0, zlo);
-        tmem_st16(ya + 128 + i0, zhi);
+        xch[L] = tmid;
+      } else {
+        double y = 0.0;
+        if (two)
+          for (int c = c_hi; c >= c_lo; --c) {
+            const int i0 = 16 * c;
+            uint32_t f[16], zlo[16], zhi[16];
+            tmem_ld16u(src + i0, f);
+            tc::mbar_wait(&bar_ib[c], ph_ib);
+#pragma unroll
+            for (int u = 15; u >= 0; --u) {
+              const int i = i0 + u;
+              const double ib = ibs[i * 128 + L];
+              const double v = fma(-(ib * ce_s[i]), y, ib * (double)__uint_as_float(f[u]));
+              y = (i < nri) ? v : y;
+              zlo[u] = (uint32_t)__double2loint(v);
+              zhi[u] = (uint32_t)__double2hiint(v);
+            }
+            tmem_st16(ya + i0, zlo);
+            tmem_st16(ya + 128 + i0, zhi);
+          }
+        xch[128 + L] = y;
+        tc::mbar_wait(&bar_ib[cm], ph_ib);                 // the meeting row's pivot
       }
       tmem_wait_st();
+      asm volatile("bar.sync %0, 64;\n" ::"r"(1 + (warp & 3)) : "memory");      // the two warps of this lane quarter
       TCS_T(8);
-      double x = 0.0;
-      for (int c = 7; c >= 0; --c) {
-        const int i0 = 16 * c;
-        uint32_t zlo[16], zhi[16];
-        tmem_ld16u(ya + i0, zlo);
-        tmem_ld16u(ya + 128 + i0, zhi);
+      double x = ibs[mid * 128 + L] * fma(-ce_s[mid], xch[128 + L], xch[L]);     // x_mid (y = 0 when there is no bottom half)
+      if (half == 0) {
+        for (int c = cm; c >= 0; --c) {
+          const int i0 = 16 * c;
+          uint32_t zlo[16], zhi[16];
+          tmem_ld16u(ya + i0, zlo);
+          tmem_ld16u(ya + 128 + i0, zhi);
 #pragma unroll
-        for (int u = 15; u >= 0; --u) {
-          const int i = i0 + u;
-          float xf = 0.f;
-          if (i < nri) {
-            const double zz = __hiloint2double((int)zhi[u], (int)zlo[u]);
-            x = fma(-(ce_s[i] * ibs[i * 128 + L]), x, zz);
-            xf = (float)x;
+          for (int u = 15; u >= 0; --u) {
+            const int i = i0 + u;
+            if (i < mid) x = fma(-(ce_s[i] * ibs[i * 128 + L]), x, __hiloint2double((int)zhi[u], (int)zlo[u]));
+            zlo[u] = __float_as_uint(i <= mid ? (float)x : 0.f);
           }
-          zlo[u] = __float_as_uint(xf);
+          tmem_st16(ya + i0, zlo);                         // x (FP32) over z's low words; split hi / lo by all warps below
         }
-        tmem_st16(ya + i0, zlo);                           // x (FP32) over z's low words; split hi / lo by all warps below
+      } else if (two) {
+        for (int c = c_lo; c <= c_hi; ++c) {
+          const int i0 = 16 * c;
+          uint32_t zlo[16], zhi[16];
+          tmem_ld16u(ya + i0, zlo);
+          tmem_ld16u(ya + 128 + i0, zhi);
+#pragma unroll
+          for (int u = 0; u < 16; ++u) {
+            const int i = i0 + u;
+            float xf = 0.f;
+            if (i < nri) {
+              x = fma(-(cw_s[i] * ibs[i * 128 + L]), x, __hiloint2double((int)zhi[u], (int)zlo[u]));
+              xf = (float)x;
+            }
+            zlo[u] = __float_as_uint(xf);
+          }
+          tmem_st16(ya + i0, zlo);
+        }
       }
       tmem_wait_st();
       tc::tc_fence_before();
       TCS_T(9);
     } else if (elected) {
       // the forward products have completed: operand tiles and the forward table are dead.  Stage the
-      // inverse pivots (rows of 128 lanes x 8 bytes, 16 rows per copy) and fetch the inverse table.
+      // inverse pivots (rows of 128 lanes x 8 bytes, 16 rows per copy; outermost chunks first, as the two
+      // sweeps consume them) and fetch the inverse table.
       tc::mbar_wait(&bar_mma, ph_mma);
-      for (int c = 0; c < 8; ++c) {
+      for (int cc = 0; cc < 8; ++cc) {
+        const int c = (cc & 1) ? 7 - (cc >> 1) : (cc >> 1);
         tc::mbar_expect_tx(&bar_ib[c], 16384);
         asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(op_a + c * 16384),
                      "l"(S.tcib + (size_t)c * 16 * 128), "r"(16384), "r"(tc::smem_u32(&bar_ib[c]))
@@ -469,14 +521,21 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
         // -dI'/dZ column for the NEXT fit, on the nodes of the compact list only (lim_mask dilated by one row;
         // everything else keeps the zero of the memset at the start of the call)
         __syncthreads();
-        float *dzc = D.dzc + (size_t)s * N;
+        float *__restrict__ dzc = D.dzc + (size_t)s * N;
         const float hz = float(0.5 / D.dz);
         const unsigned *dbits = mbits + 2 * nwords;
-#pragma unroll 2
-        for (int k = warp; k < WL.n_dil; k += nth >> 5) {
-          const int w = WL.dil[k];
+        const int nwarp = nth >> 5;
+        int k = warp;
+        int wc = k < WL.n_dil ? WL.dil[k] : 0;
+        unsigned dbc = dbits[wc];
+        while (k < WL.n_dil) {                             // word index and mask word fetched one iteration ahead
+          const int w = wc;
+          const unsigned db = dbc;
+          k += nwarp;
+          wc = k < WL.n_dil ? WL.dil[k] : 0;
+          dbc = dbits[wc];
           const int n = (w << 5) + lane;
-          if ((dbits[w] >> lane) & 1u) dzc[n] = -(G[n + nr] - G[n - nr]) * hz;     // G = 0 off the lim_mask nodes (search_lean)
+          if ((db >> lane) & 1u) dzc[n] = -(G[n + nr] - G[n - nr]) * hz;     // G = 0 off the lim_mask nodes (search_lean)
         }
       }
       TCS_T(6);

@@ -534,6 +534,40 @@ def test_small_grids_solve_stage(n, precision):
     rec.close()
 
 
+@pytest.mark.parametrize("nr", [6, 20, 33, 48, 97, 129])
+def test_tc_solve_route_any_nr(nr):
+    """Grids with N_Z = 129 take the tcgen05 solve kernel (FP32) for every N_R <= 129: tridiagonal systems of
+    length N_R - 2 on the twisted factorisation (two sweeps that meet in a row whose index + 1 is a multiple of
+    16; systems shorter than 32 rows have a single sweep).  Solve stage against the oracle's banded LU."""
+    torch = _torch()
+    from oracle.gs_solve import GSOperator, boundary_nodes
+    import paper_2601_12378_b200 as P
+    rng = np.random.default_rng(nr)
+    nz = 129
+    grid = dict(nr=nr, nz=nz, rmin=0.15, rmax=1.6, zmin=-1.5, zmax=1.5)
+    op = GSOperator(nr, nz, 0.15, 1.6, -1.5, 1.5)
+    bnd = boundary_nodes(nr, nz)
+    lim = np.zeros((nz, nr), np.uint8); lim[2:-2, 2:-2] = 1
+    M, nc = 6, 3
+    geom = dict(n_meas=M, n_coil=nc, sigma=np.ones(M), lim_r=np.array([0.5, 1.2, 0.9]), lim_z=np.array([-0.5, 0.0, 0.6]), lim_mask=lim,
+                xpt_mask=None, ip_sign=1, cold_rc=0.8, cold_zc=0.0, cold_a=0.4, cold_b=0.7)
+    tables = dict(gp=rng.normal(size=(M, nr * nz)), gc=rng.normal(size=(M, nc)), gb=rng.normal(size=(len(bnd), nr * nz)) * 1e-7,
+                  ggc=rng.normal(size=(nr * nz, nc)) * 1e-7)
+    dev = dict(grid=grid, geom=geom, tables=tables, basis=dict(n_p=1, n_ff=1, lambda_reg=0.01, relax=1.0, delz=0))
+    B = 5
+    rec = P.Reconstructor(dev, precision="fp32", max_batch=B)
+    I = (rng.uniform(0.0, 40.0, (B, nr * nz)) * lim.ravel()[None, :]).astype(np.float32)
+    pbd = rng.uniform(-0.05, 0.05, (B, len(bnd))).astype(np.float32)
+    out = torch.zeros(B, nz, nr, dtype=rec.dtype, device="cuda")
+    rec.debug_gs_solve(torch.tensor(I, device="cuda"), torch.tensor(pbd, device="cuda"), out)
+    psi = out.cpu().numpy().astype(np.float64)
+    for q in range(B):
+        edge = np.zeros(nr * nz); edge[bnd] = pbd[q].astype(np.float64)
+        ref = op.solve_current(I[q].astype(np.float64).reshape(nz, nr), edge.reshape(nz, nr))
+        assert psi_rel_err(psi[q], ref) <= PSI_TOL["fp32"], (nr, q, psi_rel_err(psi[q], ref))
+    rec.close()
+
+
 def test_large_batch_beyond_one_wave_of_row_tiles():
     """batches whose response GEMM needs more than 148 row tiles (B > 2368 at 8 rows per
     slice) must stay inside the split-K partial buffers.  B = 2500 on config 2: the 8 stored slices tiled
