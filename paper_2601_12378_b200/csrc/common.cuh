@@ -85,10 +85,30 @@ struct Dev {
   T *xn, *psi_coil, *dred, *resp, *cur, *dzc, *psi_bdry, *fhat;
   double *ytmp;                   // [B][nri][nzi]
   double *X, *Xprev;              // [B][nt]
+  float *pco;                     // [B][PCO_STRIDE] polynomial form of I'(x) = R dA P(x) + (mu0 dA / R) Q(x) of the last fit: P[0..MAX_DEG], Q[0..MAX_DEG], X_delz
   double *chi2;                   // [B]
   SearchOut *so;                  // [B]
   int *status;                    // [B]
 };
+
+constexpr int PCO_STRIDE = 2 * (PTEFIT_MAX_DEG + 1) + 2;
+
+// After a fit kernel has stored X of slice s (same warp): the P' and FF' sums of I' = J_b(x) X are polynomials in x;
+// their coefficients (FP64 sums, rounded to float) are written once here instead of being rebuilt by every consumer
+// (k_current_split, k_solve_tc).  Entry 2 (MAX_DEG + 1) = the coefficient of the vertical-shift column.
+template <typename T>
+__device__ __forceinline__ void emit_pco(const Dev<T> &D, int s, int lane) {
+  __syncwarp();
+  const double *X = D.X + (size_t)s * D.nt;
+  if (lane < 2 * (PTEFIT_MAX_DEG + 1)) {
+    const int kind = lane / (PTEFIT_MAX_DEG + 1), k = lane - kind * (PTEFIT_MAX_DEG + 1);
+    double c = 0.0;
+    for (int l = 0; l < D.npoly; ++l)
+      if (D.terms[l].kind == kind && D.terms[l].family == 0) c += X[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
+    D.pco[(size_t)s * PCO_STRIDE + lane] = float(c);
+  }
+  if (lane == 2 * (PTEFIT_MAX_DEG + 1)) D.pco[(size_t)s * PCO_STRIDE + lane] = D.has_delz ? float(X[D.nt - 1]) : 0.f;
+}
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll

@@ -281,6 +281,7 @@ __global__ void __launch_bounds__(128) k_lsq(Dev<T> D, int B) {
       if (st != 0) D.status[s] = st;
     }
   }
+  emit_pco(D, s, lane);
 }
 
 // A4, second driver: modified Gram-Schmidt QR ("Gram-Schmidt QR ... stable, slower") of the
@@ -371,6 +372,7 @@ __global__ void __launch_bounds__(32) k_lsq_mgs(Dev<T> D, int B) {
     D.chi2[s] = c2;
     if (st != 0) D.status[s] = st;
   }
+  emit_pco(D, s, lane);
 }
 
 // A5: node currents I = J_b X in amperes.  grid (ceil(N/256), B).

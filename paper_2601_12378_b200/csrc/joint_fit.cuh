@@ -144,6 +144,8 @@ __global__ void __launch_bounds__(JOINT_THREADS) k_lsq_joint(Dev<T> D, int B) {
     D.chi2[s] = tot;
     if (st != 0) D.status[s] = st;
   }
+  __syncthreads();
+  if (tid < 32) emit_pco(D, s, tid);
 }
 
 // psi_coil = G_GC I_C' with the fitted currents (Eq. 7: the coil flux follows the fit).  grid (ceil(N/256), B).

@@ -363,6 +363,7 @@ static ptefit_status build(ptefit_handle *h, Dev<T> &D, const ptefit_grid *g, co
   TRY(dev_alloc(h, &D.fhat, (size_t)B * D.nri * D.nzi));
   TRY(dev_alloc(h, &D.ytmp, (size_t)B * D.nri * D.nzi));
   TRY(dev_alloc(h, &D.X, (size_t)B * D.nt));
+  TRY(dev_alloc(h, &D.pco, (size_t)B * PCO_STRIDE));
   TRY(dev_alloc(h, &D.Xprev, (size_t)B * D.nt));
   TRY(dev_alloc(h, &D.chi2, (size_t)B));
   TRY(dev_alloc(h, &D.so, (size_t)B));

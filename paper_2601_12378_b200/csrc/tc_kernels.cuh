@@ -99,24 +99,19 @@ __global__ void __launch_bounds__(256) k_resp_reduce(Dev<float> D, TcDev Tc) {
 // grid (ceil(Kc/2048), B), block 256.
 __global__ void __launch_bounds__(256) k_current_split(Dev<float> D, TcDev Tc) {
   __shared__ float pco[2 * (PTEFIT_MAX_DEG + 1)];
-  __shared__ float xdz;
   const int s = blockIdx.y;
   const double *X = D.X + (size_t)s * D.nt;
-  if (threadIdx.x < 2 * (PTEFIT_MAX_DEG + 1)) {
-    const int kind = threadIdx.x / (PTEFIT_MAX_DEG + 1), k = threadIdx.x - kind * (PTEFIT_MAX_DEG + 1);
-    double c = 0.0;
-    for (int l = 0; l < D.npoly; ++l)
-      if (D.terms[l].kind == kind && D.terms[l].family == 0) c += X[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
-    pco[threadIdx.x] = float(c);
-  }
-  if (threadIdx.x == 32) xdz = D.has_delz ? float(X[D.nt - 1]) : 0.f;
-  __syncthreads();
+  const float *pg = D.pco + (size_t)s * PCO_STRIDE;     // polynomial form of the fitted current profile, written by the fit kernel
   constexpr int MD = PTEFIT_MAX_DEG;
   const bool lowdeg = D.maxdeg <= 4;
   float pp[5], pq[5];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) { pp[k] = pco[k]; pq[k] = pco[MD + 1 + k]; }
-  const float xd = xdz;
+  for (int k = 0; k < 5; ++k) { pp[k] = __ldg(pg + k); pq[k] = __ldg(pg + MD + 1 + k); }
+  const float xd = __ldg(pg + 2 * (MD + 1));
+  if (!lowdeg) {                                        // uniform: high-degree terms read the coefficients from shared memory
+    if (threadIdx.x < 2 * (MD + 1)) pco[threadIdx.x] = pg[threadIdx.x];
+    __syncthreads();
+  }
   const float *xs = D.xn + (size_t)s * D.N, *ds = D.dzc + (size_t)s * D.N;
   float *cs = D.cur + (size_t)s * D.N;
 #pragma unroll

@@ -195,14 +195,7 @@ k_solve_tc(const __grid_constant__ CUtensorMap mapFhi, const __grid_constant__ C
     T *G = Gb + (vec_ok ? (int)(((size_t)s * N) & 3) : 0);     // G + n is 16-byte aligned exactly when psi + n is
     __syncthreads();                                       // previous slice done with G and pb
     for (int k = tid; k < D.nbnd; k += nth) pb[k] = pbg[k];
-    if (do_search && D.has_delz && tid < 2 * (PTEFIT_MAX_DEG + 1)) {
-      const int kind = tid / (PTEFIT_MAX_DEG + 1), k = tid - kind * (PTEFIT_MAX_DEG + 1);
-      const double *Xp = D.X + (size_t)s * D.nt;
-      double c = 0.0;
-      for (int l = 0; l < D.npoly; ++l)
-        if (D.terms[l].kind == kind && D.terms[l].family == 0) c += Xp[l] * ((D.terms[l].i == k ? 1.0 : 0.0) - (D.terms[l].N == k ? 1.0 : 0.0));
-      pcoef[tid] = T(c);
-    }
+    if (do_search && D.has_delz && tid < 2 * (PTEFIT_MAX_DEG + 1)) pcoef[tid] = D.pco[(size_t)s * PCO_STRIDE + tid];   // written by the fit kernel (emit_pco)
     // ---- A. right-hand side -mu0 R I / dA with the Dirichlet data moved over, folded about the mid
     // row and written K-major (row = grid column, k = folded grid row) as hi / lo TF32 tiles.
     // Work item = one grid column n x four consecutive folded rows jj0..jj0+3 (one 16-byte chunk).
