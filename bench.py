@@ -406,6 +406,13 @@ def latency_batch1(args, torch, P):
         e0.record(); rec.reconstruct(d_b, d_ic, 1, warm_start=True); e1.record()
         torch.cuda.synchronize()
         tw.append(e0.elapsed_time(e1))
+    # the same in continue mode (warm_start = 2: the handle's own previous output is the start, its search is not repeated)
+    tc2 = []
+    for _ in range(50):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); rec.reconstruct(d_b, d_ic, 1, warm_start=2); e1.record()
+        torch.cuda.synchronize()
+        tc2.append(e0.elapsed_time(e1))
     # flux-surface post-processing of the paper's timing (33 profile points; Sec. II.E): 33 levels x 128
     # chords, 10 bisections, three Q integrals, q profile, LCFS geometry -- a separate call (ptefit_flux_surfaces)
     for _ in range(3):
@@ -439,18 +446,18 @@ def latency_batch1(args, torch, P):
     stat = torch.zeros(n_stream, dtype=torch.int32, device="cuda")
     evs[0].record()
     for q in range(n_stream):
-        rec.reconstruct(b_all[q:q + 1], ic_all[q:q + 1], 1, warm_start=True)
+        rec.reconstruct(b_all[q:q + 1], ic_all[q:q + 1], 1, warm_start=2)      # continue mode: slice q starts from what slice q - 1 left
         evs[q + 1].record()
         stat[q:q + 1].copy_(rec.status[0:1], non_blocking=True)    # outside the event pair of slice q, inside that of q + 1
     torch.cuda.synchronize()
     st = np.array([evs[q].elapsed_time(evs[q + 1]) for q in range(n_stream)]) * 1e3
     stream = dict(slices=n_stream, us_mean=float(st.mean()), us_p50=float(np.percentile(st, 50)), us_p99=float(np.percentile(st, 99)),
                   us_max=float(st.max()), status_ok=int((stat == 0).sum().item()),
-                  note="one warm-started Picard iteration per slice, back-to-back launches, no post-processing")
+                  note="one Picard iteration per slice continuing the previous slice (warm_start = 2), back-to-back launches, no post-processing")
     rec.close()
     return dict(workload="cfg3", streaming=stream, us_per_slice=1e3 * float(np.median(ts)), us_min=1e3 * float(min(ts)), n_iter=c["n_iter"],
                 us_per_iteration=1e3 * float(np.median(ts)) / c["n_iter"],
-                us_one_warm_iteration=1e3 * float(np.median(tw)), us_flux_surfaces=us_flux,
+                us_one_warm_iteration=1e3 * float(np.median(tw)), us_one_continue_iteration=1e3 * float(np.median(tc2)), us_flux_surfaces=us_flux,
                 us_warm_iteration_plus_flux_surfaces=1e3 * float(np.median(tw)) + us_flux,
                 launches_per_call=n, paper_context="0.268 ms/slice at 129x129 on the paper's GPU (PAPER.md:175), other hardware")
 

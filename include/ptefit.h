@@ -131,7 +131,13 @@ ptefit_status ptefit_reconstruct(ptefit_handle *h, int batch,
     const void *d_ic,       /* [batch][n_coil]  real: coil + eddy currents I_C                  */
     int n_iter, int warm_start, /* warm_start = 1: d_psi holds the starting flux, and the coefficients
                                    of this handle's previous call seed the vertical-shift column of the
-                                   first iteration (slice q continues slice q of that call)         */
+                                   first iteration (slice q continues slice q of that call).
+                                   warm_start = 2 ("continue", the streaming mode of PAPER.md:158): as 1, and
+                                   d_psi still holds exactly what this handle's previous ptefit_reconstruct
+                                   call (n_iter >= 1, batch >= this one) returned: the search of the starting
+                                   flux and the rebuild of the vertical-shift column are skipped, because that
+                                   call's last kernel left both behind.  PTEFIT_ERR_INVALID_ARG if there is no
+                                   such call (or a ptefit_debug_* hook ran since); needs n_iter >= 1.      */
     void *d_psi,            /* [batch][nz][nr]  real, in/out: poloidal flux per radian          */
     void *d_coeffs,         /* [batch][n_terms] real: X of the last fit (Eq. 11)                */
     int *d_axis_ij,         /* [batch][2] (i, j) of the axis node                               */

@@ -41,6 +41,7 @@ struct ptefit_handle {
   std::vector<void *> allocs;
   std::string error;
   int launches = 0;
+  int state_batch = 0;                  // slices whose (xn, delz column, X) are those of the last ptefit_reconstruct call (warm_start = 2)
   bool tc = false;                      // tensor-core contractions usable (FP32, 3xTF32 mode)
   TcDev Tc{};
   const float *gp_hi = nullptr, *gp_lo = nullptr, *gb_hi = nullptr, *gb_lo = nullptr;

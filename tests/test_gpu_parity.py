@@ -650,6 +650,46 @@ def test_warm_start_and_ragged_batch_fp32_tc_path():
     rec.close()
 
 
+@pytest.mark.parametrize("name,precision", [("cfg3", "fp32"), ("cfg2", "fp64")])
+def test_continue_mode_streaming(name, precision):
+    """warm_start = 2 (continue the handle's previous call: the search of the starting flux and the rebuild of
+    the vertical-shift column are skipped because the previous call's last kernel left them behind): six
+    one-iteration calls against the oracle continued the same way, and against warm_start = 1 on a second
+    handle (same flux, the column rebuilt by another kernel: equal to FP32 / FP64 rounding).  Misuse is rejected."""
+    torch = _torch()
+    import paper_2601_12378_b200 as P
+    dev, sl = cached_case(name, 2)
+    dv, b, ic = round_inputs(dev, sl, precision)
+    od = oracle_device(dv)
+    n0 = 8
+    recs = [_rec(dev, precision, 2), _rec(dev, precision, 2)]
+    db = torch.tensor(b, dtype=recs[0].dtype, device="cuda"); dic = torch.tensor(ic, dtype=recs[0].dtype, device="cuda")
+    with pytest.raises(P.PtefitError, match="continues the previous"):
+        recs[0].reconstruct(db, dic, 1, warm_start=2)              # nothing to continue yet
+    for mode, rec in zip((2, 1), recs):
+        rec.reconstruct(db, dic, n0)
+        for _ in range(6):
+            rec.reconstruct(db, dic, 1, warm_start=mode)
+    torch.cuda.synchronize()
+    o2, o1 = _gpu_out(recs[0], 2), _gpu_out(recs[1], 2)
+    tol = PSI_TOL[precision]
+    for q in range(2):
+        o = reconstruct(od, b[q], ic[q], n0)
+        for _ in range(6):
+            o = reconstruct(od, b[q], ic[q], 1, psi0=o["psi"], X0=o["X"])
+        assert o["status"] == 0 and int(o2["status"][q]) == 0 and int(o1["status"][q]) == 0
+        assert psi_rel_err(o2["psi"][q], o["psi"]) <= tol, (q, psi_rel_err(o2["psi"][q], o["psi"]))
+        assert psi_rel_err(o2["psi"][q], o1["psi"][q].astype(np.float64)) <= tol
+        assert tuple(o2["axis_ij"][q]) == tuple(o["srch"]["axis"][:2]) == tuple(o1["axis_ij"][q])
+        assert np.allclose(o2["coeffs"][q], o1["coeffs"][q], rtol=1e-3 if precision == "fp32" else 1e-8, atol=0)
+    # a larger batch than the previous call covered, and a test hook in between, invalidate the state
+    recs[0].reconstruct(db[:1], dic[:1], 1, warm_start=2)
+    with pytest.raises(P.PtefitError, match="continues the previous"):
+        recs[0].reconstruct(db, dic, 1, warm_start=2)
+    for r in recs:
+        r.close()
+
+
 def test_cfg4_every_slice_of_the_batch_against_oracle():
     """BASELINE config 4 exactly as bench.py times it (512 distinct designed slices, max_batch 512, 20
     iterations): EVERY slice against the oracle (about 80 s of oracle time), with the figures printed."""
